@@ -1,0 +1,304 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the MHD hot path (BASELINE.json metric) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--dtype f64|f32] [--n 512] [--impl ours|reference]
+
+A "step" is one full 2N-RK3 time step (3 fused substep kernels + the forcing-table kernel) of the
+whole hot path over one synthetic box.  Default workload: BASELINE config 4 (512^3, nu = eta = 5e-4,
+helical forcing k_f = 3, f0 = 0.02, seeded solenoidal u of rms 0.1, weak Gaussian A, fixed CFL dt).
+Prints ONE JSON line (see DESIGN.md "Measurement" for every key).
+
+N > 1: the path does not shard yet (one GPU only): each rank advances an
+independent replica of the box, value = N boxes' cells / max-over-ranks time ("replicas only").
+"""
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "MHD cell-updates/s per RK3 step"
+UNIT = "cell-updates/s"
+WORDS_PER_CELL_STEP = 56           # 14 (substep 0) + 21 + 21, DESIGN.md "algorithmic bytes"
+TWO_PI3 = (2 * math.pi,) * 3
+CONFIGS = {                        # BASELINE.json configs 3-5 (index = position in configs[])
+    256: dict(seed=1003, nu=1e-3, sigma=0.0, name="config3_256^3"),
+    512: dict(seed=1004, nu=5e-4, sigma=1.0, name="config4_512^3"),
+    1024: dict(seed=1005, nu=2.5e-4, sigma=0.0, name="config5_1024^3"),
+}
+
+
+def workload(n):
+    return CONFIGS.get(n, dict(seed=1000 + n, nu=5e-4 * 512 / n, sigma=1.0, name="box_%d^3" % n))
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def committed_traffic(dtype):
+    """DRAM bytes per substep launch from the committed ncu --set full summary, or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get(dtype)
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index = index
+        self.samples = []
+        self.reasons = set()
+        self.max_mhz = None
+        self._stop_evt = threading.Event()
+
+    def run(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM)
+            names = {
+                pynvml.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                pynvml.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                pynvml.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                pynvml.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                pynvml.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake",
+            }
+            while not self._stop_evt.is_set():
+                self.samples.append(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                r = pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                self._stop_evt.wait(0.02)
+        except Exception as e:                      # never let the sampler kill the bench
+            self.reasons.add("sampler_error:%s" % type(e).__name__)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def time_oracle(n_sample, cfg, steps, warmup=0):
+    """The oracle as it stands, timed on the host cores on a bounded sample of the workload."""
+    from oracle import forcing as of, mhd_c
+    from paper_2012_08758_b200 import inputs
+    state = inputs.solenoidal_state(n_sample, cfg["seed"])
+    nu = cfg["nu"]
+    st = mhd_c.Stepper(state, TWO_PI3, nu, nu, 1.0)
+    h = 2 * math.pi / n_sample
+    umax = float(np.sqrt((state[1:4] ** 2).sum(axis=0).max()))
+    dt = min(0.4 * h / (umax + 1.0), 0.25 * h * h / nu)
+    times = []
+    for s in range(warmup + steps):
+        f = of.forcing_from_draws(*inputs.counter_uniforms(cfg["seed"] + 7, s), 3, cfg["sigma"], dt, 0.02, 1.0)
+        t0 = time.perf_counter()
+        st.step(dt, f)
+        if s >= warmup:
+            times.append(time.perf_counter() - t0)
+    return n_sample ** 3 / float(np.mean(times)), float(np.mean(times)), mhd_c.max_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = workload(args.n)
+    n_sample = min(args.n, args.ref_sample)
+    value, sec, cores = time_oracle(n_sample, cfg, args.steps, args.warmup)
+    sample = "each step = one RK3 step of the C oracle on a %d^3 box of the %s recipe" % (n_sample, cfg["name"])
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "grid": [args.n] * 3, "sample_grid": [n_sample] * 3},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    from paper_2012_08758_b200 import binding, inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    n = args.n
+    cfg = workload(n)
+    nu = cfg["nu"]
+
+    def bench_dtype(dtype_name, do_e2e):
+        dtype = binding.AC_F64 if dtype_name == "f64" else binding.AC_F32
+        npdt = np.float64 if dtype_name == "f64" else np.float32
+        es = 8 if dtype_name == "f64" else 4
+        ctx = binding.Context((n, n, n), TWO_PI3, dtype, nu=nu, eta=nu, cs=1.0, k_f=3.0, helicity=cfg["sigma"],
+                              device="cuda:%d" % local_rank)
+        ctx.ac_set_variant(args.variant)
+        host = torch.from_numpy(inputs.solenoidal_state(n, cfg["seed"] + rank).astype(npdt)).pin_memory()
+        ctx.ac_load_state(host)
+        dt = ctx.ac_reduce()["dt_cfl"]
+        forcings = [ctx.ac_make_forcing(cfg["seed"] + 7, s, dt, 0.02) for s in range(args.warmup + args.steps)]
+        for s in range(args.warmup):
+            ctx.ac_step(dt, forcings[s])
+        ctx.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+        l0 = ctx.ac_launch_count()
+        ev[0].record(ctx.stream)
+        for s in range(args.steps):
+            ctx.ac_step(dt, forcings[args.warmup + s])
+            ev[s + 1].record(ctx.stream)
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        clocks = sampler.stop()
+        launches = ctx.ac_launch_count() - l0
+        total_ms = ev[0].elapsed_time(ev[-1])
+        per = np.array([ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)])
+        if dist is not None:
+            t = torch.tensor([total_ms], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            total_ms = float(t.item())
+        diag = ctx.ac_reduce()
+        ms_per_step = total_ms / args.steps
+        value = world * n ** 3 / (ms_per_step * 1e-3)
+        peak, peak_src = measured_peak()
+        alg_bytes_launch = WORDS_PER_CELL_STEP / 3.0 * es * n ** 3         # average over the 3 substep launches
+        launch_ms = ms_per_step / 3.0
+        achieved = alg_bytes_launch / (launch_ms * 1e-3) / 1e9
+        res = {
+            "value": value, "ms_per_step": ms_per_step, "ms_median": float(np.median(per)),
+            "ms_p90": float(np.percentile(per, 90)), "dt": dt, "launches": launches, "clocks": clocks,
+            "diag": {k: diag[k] for k in ("urms", "brms", "nonfinite")},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": committed_traffic(dtype_name), "peak_source": peak_src,
+                         "kernel": "substep (avg of the 3 launches of a step)",
+                         "algorithmic_bytes_per_launch": alg_bytes_launch},
+        }
+        if do_e2e:
+            # end to end through the C ABI with HOST buffers: H2D of the whole state, one step, D2H of the state
+            out = torch.empty_like(host)
+            k_e2e = max(1, min(args.steps, args.e2e_steps))
+            ctx.ac_load_state(host)
+            ctx.ac_step(dt, forcings[0])
+            ctx.ac_store_state(out)                        # untimed warm-up of the copy path
+            torch.cuda.synchronize()
+            if dist is not None:
+                dist.barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(ctx.stream)
+            for s in range(k_e2e):
+                ctx.ac_load_state(host)
+                ctx.ac_step(dt, forcings[s])
+                ctx.ac_store_state(out)
+            e1.record(ctx.stream)
+            torch.cuda.synchronize()
+            e2e_ms = e0.elapsed_time(e1) / k_e2e
+            if dist is not None:
+                t = torch.tensor([e2e_ms], device="cuda")
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                e2e_ms = float(t.item())
+            nbytes = 7 * n ** 3 * es
+            res["e2e"] = {"value": world * n ** 3 / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+                          "d2h_bytes_per_step": nbytes, "ms_per_step": e2e_ms, "steps": k_e2e,
+                          "what": "ac_load_state(pinned host) + ac_step + ac_store_state(pinned host) per step"}
+            del out
+        ctx.ac_free()
+        del ctx, host
+        torch.cuda.empty_cache()
+        return res
+
+    main = bench_dtype(args.dtype, True)
+    other_name = "f32" if args.dtype == "f64" else "f64"
+    other = bench_dtype(other_name, False) if not args.single_dtype else None
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        n_s = min(n, args.ref_sample)
+        v, sec, cores = time_oracle(n_s, cfg, 1)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "1 RK3 step of the C oracle (fp64, OpenMP) on a %d^3 box of the same recipe; %.1f s" % (n_s, sec)}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+            "config": {"workload": cfg["name"], "grid": [n, n, n], "nu": nu, "eta": nu, "helicity": cfg["sigma"],
+                       "k_f": 3, "f0": 0.02, "dt": main["dt"], "l2": "state (14 arrays) far larger than L2; no flush needed",
+                       "parallelism": "replicas only" if world > 1 else "single GPU", "variant": args.variant},
+            "ms_median": main["ms_median"], "ms_p90": main["ms_p90"],
+            "roofline": main["roofline"], "cpu_baseline": cpu, "e2e": main.get("e2e"),
+            "gpu_launches": main["launches"], "clocks": main["clocks"], "diag": main["diag"],
+            "paper_context": {"astaroth_4xV100_fp64_cell_updates_per_s": 1.0 / 0.65e-9,
+                              "pencil_40cores_cell_updates_per_s": 1.0 / 23.17e-9, "source": "PAPER.md:535"},
+        }
+        if other is not None:
+            line["also"] = {"dtype": other_name, "value": other["value"], "ms_per_step": other["ms_per_step"],
+                            "ms_median": other["ms_median"], "roofline": other["roofline"], "clocks": other["clocks"],
+                            "gpu_launches": other["launches"]}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--n", type=int, default=512)
+    ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--single-dtype", action="store_true", help="skip the second precision")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-sample", type=int, default=128, help="box size of the bounded oracle sample")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

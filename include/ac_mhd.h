@@ -1,0 +1,154 @@
+/*
+ * ac_mhd.h - C ABI of the B200-native MHD time-stepping library (libac_mhd.so).
+ *
+ * The library advances the state (ln rho, u, A) of compressible isothermal resistive MHD on a
+ * triply periodic grid by full 2N-RK3 time steps and reduces rms/max diagnostics.  Everything on
+ * the path runs in hand-written sm_100a CUDA kernels; there is no CPU fallback: every entry point
+ * that needs the device returns AC_ECUDA if there is none.
+ *
+ * What is computed (citations: /root/reference/PAPER.md line numbers; "G<n>" = reading listed
+ * in DESIGN.md where the paper is silent):
+ *   Eq. 1  D ln rho/Dt = -div u
+ *   Eq. 2  Du/Dt = -cs^2 grad ln rho + j x B / rho
+ *                  + nu [lap u + 1/3 grad div u + 2 S.grad ln rho] + f
+ *   Eq. 3  dA/dt = u x B + eta lap A     (B = curl A, j = curl B, mu0 = 1)
+ *   Eq. 4  f(x) = Re{N f_k exp[i k.x + i phi]}, Eq. 5 N, Eq. 6 f_k
+ *   6th-order central finite differences, stencil radius 3 (G1-G3)
+ *   3rd-order 2N-storage Runge-Kutta, two state buffers swapped per substep (G7)
+ *   runtime reductions ("global averages")
+ *
+ * Conventions
+ *   - Fields, in this order everywhere: lnrho, ux, uy, uz, ax, ay, az  (AC_NFIELDS = 7).
+ *   - A caller-visible field is a dense array of nz*ny*nx elements, x fastest:
+ *       index = x + nx*(y + ny*z),  element type = the context's dtype (float or double).
+ *   - Cell (x, y, z) sits at position (x*lx/nx, y*ly/ny, z*lz/nz).
+ *   - All functions return 0 (AC_OK) or a negative ac_status; no exceptions cross the ABI.
+ *   - Device work is enqueued on the CUDA stream given to ac_init and is asynchronous unless
+ *     stated otherwise.  A context must be used from one host thread at a time.
+ *   - Ownership: the library owns everything it allocates; the caller owns every pointer it
+ *     passes in, and may free or reuse it as soon as the call returns, except the workspace
+ *     given to ac_init, which must outlive the context.
+ */
+#ifndef AC_MHD_H
+#define AC_MHD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define AC_NFIELDS 7
+
+typedef struct ac_ctx ac_ctx; /* opaque */
+
+typedef enum { AC_F32 = 0, AC_F64 = 1 } ac_dtype;
+
+typedef enum {
+    AC_OK = 0,
+    AC_EINVAL = -1, /* NULL pointer, bad grid (n < 8, nx % 4 != 0), non-positive L or cs, negative nu/eta, bad dt */
+    AC_ENOMEM = -2, /* device or host allocation failed / workspace too small */
+    AC_ECUDA = -3,  /* CUDA error (sticky); text from ac_strerror(AC_ECUDA) on the same thread */
+    AC_ESTATE = -4  /* ac_step / ac_reduce / ac_store_state before ac_load_state */
+} ac_status;
+
+/* Periodic box: n cells and side length per axis; spacing h_a = l_a / n_a (l = 2 pi). */
+typedef struct {
+    int nx, ny, nz;
+    double lx, ly, lz;
+} ac_grid;
+
+/* Forcing of one time step (Eq. 4), N of Eq. 5 folded into re, im:
+ *   f(x) = re * cos(k.x + phase) - im * sin(k.x + phase).
+ * k is in radians per unit length (integer components for l = 2 pi). */
+typedef struct {
+    double k[3];
+    double phase;
+    double re[3];
+    double im[3];
+} ac_forcing;
+
+/* Diagnostics (G18): rms = sqrt(mean over cells of |v|^2), max of |v|.
+ * B = curl A (+ external field).  dt_cfl per G15.  nonfinite != 0 if any reduced value is NaN/Inf. */
+typedef struct {
+    double urms, umax, brms, bmax;
+    double lnrho_min, lnrho_max;
+    double dt_cfl;
+    int nonfinite;
+} ac_diag;
+
+/* Bytes of device memory a context needs for this grid and dtype: 2 x 7 ghost-padded field
+ * arrays (the two state buffers of PAPER.md:143; the 2N register lives implicitly in their
+ * difference) plus forcing tables and reduction scratch.  Returns 0 for an invalid grid. */
+size_t ac_workspace_bytes(const ac_grid* grid, ac_dtype dtype);
+
+/* Create a context.
+ *   nu, eta, cs        viscosity, magnetic diffusivity, isothermal sound speed
+ *   k_f, helicity      forcing shell centre and sigma in [0, 1]; used only by
+ *                      ac_make_forcing / ac_forcing_from_draws
+ *   workspace_dev      device pointer to at least ac_workspace_bytes() bytes, 256-byte aligned,
+ *                      or NULL to let the library cudaMalloc (and free in ac_free)
+ *   cuda_stream        a cudaStream_t (as void*), or NULL for the legacy default stream
+ * Errors: AC_EINVAL, AC_ENOMEM, AC_ECUDA (no device / not sm_100). */
+int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double eta, double cs,
+            double k_f, double helicity, void* workspace_dev, void* cuda_stream);
+
+/* Copy the 7 fields in (dense caller layout -> padded device layout, ghost zones filled by
+ * periodic wrap: the "local boundary transfer" of PAPER.md:153).  src_on_device: 0 = host
+ * pointers (pinned memory makes the copy asynchronous), 1 = device pointers.  The caller may
+ * reuse its buffers when the call returns only if they are pageable host memory or after
+ * synchronising the stream. */
+int ac_load_state(ac_ctx* ctx, const void* const fields[AC_NFIELDS], int src_on_device);
+
+/* Copy the current state out into 7 dense arrays.  Host destinations: the call synchronises the
+ * stream before returning.  Device destinations: asynchronous on the stream. */
+int ac_store_state(ac_ctx* ctx, void* const fields[AC_NFIELDS], int dst_on_device);
+
+/* One full RK3 time step = 3 fused substep kernels (S1-S8 of DESIGN.md), asynchronous.
+ * forcing == NULL: no forcing.  The same forcing parameters are used in all 3 substeps (G8).
+ * Errors: AC_EINVAL (dt <= 0 or non-finite), AC_ESTATE, AC_ECUDA. */
+int ac_step(ac_ctx* ctx, double dt, const ac_forcing* forcing);
+
+/* rms/max reductions of |u| and |B| and min/max of ln rho over the current state, and the CFL
+ * time step dt = min(C_u h/(umax + cs), C_nu h^2/max(nu, eta)) (G15).  Deterministic (fixed
+ * two-stage tree, no floating-point atomics).  Synchronises the stream. */
+int ac_reduce(ac_ctx* ctx, ac_diag* out);
+
+/* Host helpers for Eq. 4-6 (no device work).
+ * ac_forcing_from_draws: u1, u2, u3 in [0, 1) choose the shell vector (index floor(u1*len) into
+ *   the lexicographically sorted shell k_f - 1/2 <= |k| <= k_f + 1/2, G11), the phase
+ *   (-pi + 2 pi u2) and the angle of e-hat around k (2 pi u3, G9); amplitude N = f0 cs sqrt(|k| cs/dt).
+ * ac_make_forcing: the same with u_i = (splitmix64(splitmix64(seed) ^ (3*step + i)) >> 11) * 2^-53. */
+int ac_forcing_from_draws(const ac_ctx* ctx, double u1, double u2, double u3, double dt, double f0,
+                          ac_forcing* out);
+/* The same without a context (pure host arithmetic, usable on a machine without a GPU):
+ * k_f, helicity (sigma), cs and the box as given to ac_init.  Errors: AC_EINVAL. */
+int ac_forcing_params(double k_f, double helicity, double cs, const ac_grid* grid, double u1, double u2, double u3,
+                      double dt, double f0, ac_forcing* out);
+int ac_make_forcing(const ac_ctx* ctx, uint64_t seed, uint64_t step, double dt, double f0, ac_forcing* out);
+
+/* Optional knobs.  ac_set_bext: uniform external field added to curl A in j x B, u x B and the
+ * |B| diagnostics (test hook for the Alfven-wave check, G16; default 0).  ac_set_cfl: C_u, C_nu
+ * (defaults 0.4, 0.25).  ac_set_variant: substep kernel variant (0 = default/fastest,
+ * others documented in DESIGN.md; AC_EINVAL if unknown). */
+int ac_set_bext(ac_ctx* ctx, const double b[3]);
+int ac_set_cfl(ac_ctx* ctx, double c_u, double c_nu);
+int ac_set_variant(ac_ctx* ctx, int variant);
+
+/* Number of kernels this context has launched so far (for the bench's gpu_launches). */
+long long ac_launch_count(const ac_ctx* ctx);
+
+/* Destroy the context (ac_free(NULL) is a no-op).  Synchronises the stream first. */
+void ac_free(ac_ctx* ctx);
+
+/* Static text for a status; for AC_ECUDA the last CUDA error text seen on this thread. */
+const char* ac_strerror(int status);
+
+/* Library version string, e.g. "ac_mhd 0.1 sm_100a". */
+const char* ac_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AC_MHD_H */

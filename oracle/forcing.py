@@ -71,8 +71,10 @@ def normalisation(kabs, dt, f0, cs):
     return f0 * cs * math.sqrt(kabs * cs / dt)
 
 
-def forcing_from_draws(u1, u2, u3, k_f, sigma, dt, f0, cs):
-    """(k[3], phase, re[3], im[3]) with re + i im = N f_k, for the three uniforms of this step."""
+def forcing_from_draws(u1, u2, u3, k_f, sigma, dt, f0, cs, lengths=(2.0 * math.pi,) * 3):
+    """(k[3], phase, re[3], im[3]) with re + i im = N f_k, for the three uniforms of this step.
+    The integer shell vector counts periods per box side; the returned k is in radians per unit
+    length, k_a * 2 pi / L_a (equal to the integers for the paper's L = 2 pi)."""
     sh = shell(k_f)
     idx = min(int(math.floor(u1 * len(sh))), len(sh) - 1)
     k = np.array(sh[idx], dtype=np.float64)
@@ -83,4 +85,5 @@ def forcing_from_draws(u1, u2, u3, k_f, sigma, dt, f0, cs):
     fk = f_k(k, ehat, sigma)
     n = normalisation(math.sqrt(k @ k), dt, f0, cs)
     amp = n * fk
-    return (k, phase, amp.real.copy(), amp.imag.copy())
+    k_phys = k * (2.0 * math.pi / np.asarray(lengths, dtype=np.float64))
+    return (k_phys, phase, amp.real.copy(), amp.imag.copy())

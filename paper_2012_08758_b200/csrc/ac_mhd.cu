@@ -1,0 +1,502 @@
+// Host side of the C ABI declared in include/ac_mhd.h.  Argument checks, memory carving, kernel
+// launches, the Eq. 4-6 host helpers.  No torch, no exceptions across the boundary.
+#include "../../include/ac_mhd.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <array>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "kernels.cuh"
+#include "layout.cuh"
+#include "mhd_cell.cuh"
+
+namespace {
+
+thread_local char g_cuda_err[256] = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t e, const char* what) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "CUDA error in %s: %s", what, cudaGetErrorString(e));
+    return AC_ECUDA;
+}
+
+#define AC_CUDA(call)                                        \
+    do {                                                     \
+        cudaError_t e__ = (call);                            \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+    } while (0)
+
+// stencil weights (G1, G2) and RK coefficients (G7)
+const double W1[3] = {3.0 / 4.0, -3.0 / 20.0, 1.0 / 60.0};
+const double W2_0 = -49.0 / 18.0;
+const double W2[3] = {3.0 / 2.0, -3.0 / 20.0, 1.0 / 90.0};
+const double WM[3] = {3.0 / 8.0, -3.0 / 80.0, 1.0 / 360.0};
+const double RK_ALPHA[3] = {0.0, -5.0 / 9.0, -153.0 / 128.0};
+const double RK_BETA[3] = {1.0 / 3.0, 15.0 / 16.0, 8.0 / 15.0};
+
+const int RED_BLOCKS = 148 * 8;
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+bool grid_ok(const ac_grid* g) {
+    if (!g) return false;
+    if (g->nx < 8 || g->ny < 8 || g->nz < 8) return false;
+    if (g->nx % 4 != 0) return false;
+    if (!(g->lx > 0.0) || !(g->ly > 0.0) || !(g->lz > 0.0)) return false;
+    if (!std::isfinite(g->lx) || !std::isfinite(g->ly) || !std::isfinite(g->lz)) return false;
+    return true;
+}
+
+size_t elem_size(ac_dtype d) { return d == AC_F64 ? 8 : 4; }
+
+struct Carve {
+    size_t field_bytes, ftab_off, partial_off, result_off, total;
+};
+
+Carve carve(const ac::Layout& L, ac_dtype d) {
+    Carve c;
+    c.field_bytes = L.field * elem_size(d);
+    size_t off = 2 * AC_NFIELDS * c.field_bytes;
+    c.ftab_off = off;
+    off += align_up((size_t)2 * (L.nx + L.ny + L.nz) * elem_size(d), 256);
+    c.partial_off = off;
+    off += align_up(sizeof(ac::RedVals) * RED_BLOCKS, 256);
+    c.result_off = off;
+    off += 256;
+    c.total = off;
+    return c;
+}
+
+}  // namespace
+
+struct ac_ctx {
+    ac_grid grid;
+    ac_dtype dtype;
+    double nu, eta, cs, k_f, helicity;
+    double bext[3];
+    double c_u, c_nu;
+    int variant;
+    ac::Layout L;
+    Carve cv;
+    char* ws;
+    bool owns_ws;
+    cudaStream_t stream;
+    int cur;  // which of the two state buffers holds the current state
+    bool loaded;
+    long long launches;
+    ac::RedVals* host_result;  // pinned
+    std::vector<std::array<int, 3>>* shell;
+
+    void* field_ptr(int buf, int q) const { return ws + ((size_t)buf * AC_NFIELDS + q) * cv.field_bytes; }
+};
+
+namespace {
+
+template <typename T>
+void fill_coeffs(const ac_ctx* ctx, ac::Coeffs<T>& c) {
+    const double h[3] = {ctx->grid.lx / ctx->grid.nx, ctx->grid.ly / ctx->grid.ny, ctx->grid.lz / ctx->grid.nz};
+    for (int a = 0; a < 3; a++) {
+        for (int m = 0; m < 3; m++) {
+            c.c1[a][m] = (T)(W1[m] / h[a]);
+            c.c2[a][m] = (T)(W2[m] / (h[a] * h[a]));
+        }
+        c.c20[a] = (T)(W2_0 / (h[a] * h[a]));
+    }
+    const int pa[3] = {0, 0, 1}, pb[3] = {1, 2, 2};
+    for (int p = 0; p < 3; p++)
+        for (int m = 0; m < 3; m++) c.cm[p][m] = (T)(WM[m] / (h[pa[p]] * h[pb[p]]));
+}
+
+template <typename T>
+int load_state_t(ac_ctx* ctx, const void* const fields[AC_NFIELDS], int src_on_device) {
+    const ac::Layout& L = ctx->L;
+    const size_t dense_bytes = (size_t)L.nx * L.ny * L.nz * sizeof(T);
+    dim3 blk(64, 4, 1);
+    dim3 grd((L.nx + 2 * ac::R + blk.x - 1) / blk.x, (L.ny + 2 * ac::R + blk.y - 1) / blk.y, L.nz + 2 * ac::R);
+    for (int q = 0; q < AC_NFIELDS; q++) {
+        T* dst = (T*)ctx->field_ptr(0, q);
+        const T* src;
+        if (src_on_device) {
+            src = (const T*)fields[q];
+        } else {
+            // stage the dense field in the second state buffer, whose contents are dead between steps
+            T* stage = (T*)ctx->field_ptr(1, q);
+            AC_CUDA(cudaMemcpyAsync(stage, fields[q], dense_bytes, cudaMemcpyHostToDevice, ctx->stream));
+            src = stage;
+        }
+        ac::pack_kernel<T><<<grd, blk, 0, ctx->stream>>>(src, dst, L);
+        ctx->launches++;
+    }
+    AC_CUDA(cudaGetLastError());
+    ctx->cur = 0;
+    ctx->loaded = true;
+    return AC_OK;
+}
+
+template <typename T>
+int store_state_t(ac_ctx* ctx, void* const fields[AC_NFIELDS], int dst_on_device) {
+    const ac::Layout& L = ctx->L;
+    const size_t dense_bytes = (size_t)L.nx * L.ny * L.nz * sizeof(T);
+    dim3 blk(64, 4, 1);
+    dim3 grd((L.nx + blk.x - 1) / blk.x, (L.ny + blk.y - 1) / blk.y, L.nz);
+    for (int q = 0; q < AC_NFIELDS; q++) {
+        const T* src = (const T*)ctx->field_ptr(ctx->cur, q);
+        if (dst_on_device) {
+            ac::unpack_kernel<T><<<grd, blk, 0, ctx->stream>>>(src, (T*)fields[q], L);
+        } else {
+            T* stage = (T*)ctx->field_ptr(1 - ctx->cur, q);
+            ac::unpack_kernel<T><<<grd, blk, 0, ctx->stream>>>(src, stage, L);
+            AC_CUDA(cudaMemcpyAsync(fields[q], stage, dense_bytes, cudaMemcpyDeviceToHost, ctx->stream));
+        }
+        ctx->launches++;
+    }
+    AC_CUDA(cudaGetLastError());
+    if (!dst_on_device) AC_CUDA(cudaStreamSynchronize(ctx->stream));
+    return AC_OK;
+}
+
+template <typename T>
+int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
+    const ac::Layout& L = ctx->L;
+    ac::SubstepArgs<T> a;
+    a.L = L;
+    fill_coeffs<T>(ctx, a.c);
+    a.p.nu = (T)ctx->nu;
+    a.p.eta = (T)ctx->eta;
+    a.p.cs2 = (T)(ctx->cs * ctx->cs);
+    for (int i = 0; i < 3; i++) a.p.bext[i] = (T)ctx->bext[i];
+    a.p.has_forcing = forcing ? 1 : 0;
+    for (int i = 0; i < 3; i++) {
+        a.p.fre[i] = forcing ? (T)forcing->re[i] : T(0);
+        a.p.fim[i] = forcing ? (T)forcing->im[i] : T(0);
+    }
+    a.ftab = (const T*)(ctx->ws + ctx->cv.ftab_off);
+    if (forcing) {
+        const int n = L.nx + L.ny + L.nz;
+        ac::forcing_tables_kernel<T><<<(n + 255) / 256, 256, 0, ctx->stream>>>(
+            (T*)(ctx->ws + ctx->cv.ftab_off), L.nx, L.ny, L.nz, forcing->k[0], forcing->k[1], forcing->k[2],
+            ctx->grid.lx / L.nx, ctx->grid.ly / L.ny, ctx->grid.lz / L.nz, forcing->phase);
+        ctx->launches++;
+    }
+    for (int s = 0; s < 3; s++) {
+        a.p.substep = s;
+        a.p.rk_a = (s == 0) ? T(0) : (T)(RK_BETA[s] * RK_ALPHA[s] / RK_BETA[s - 1]);
+        a.p.rk_b = (T)(RK_BETA[s] * dt);
+        for (int q = 0; q < AC_NFIELDS; q++) {
+            a.in[q] = (const T*)ctx->field_ptr(ctx->cur, q);
+            a.out[q] = (T*)ctx->field_ptr(1 - ctx->cur, q);
+        }
+        {
+            dim3 blk(32, 4, 2);
+            dim3 grd((L.nx + blk.x - 1) / blk.x, (L.ny + blk.y - 1) / blk.y, (L.nz + blk.z - 1) / blk.z);
+            ac::substep_direct_kernel<T><<<grd, blk, 0, ctx->stream>>>(a);
+        }
+        ctx->launches++;
+        ctx->cur = 1 - ctx->cur;
+    }
+    AC_CUDA(cudaGetLastError());
+    return AC_OK;
+}
+
+template <typename T>
+int reduce_t(ac_ctx* ctx, ac_diag* out) {
+    const ac::Layout& L = ctx->L;
+    ac::ReduceArgs<T> a;
+    a.L = L;
+    const double h[3] = {ctx->grid.lx / L.nx, ctx->grid.ly / L.ny, ctx->grid.lz / L.nz};
+    for (int ax = 0; ax < 3; ax++)
+        for (int m = 0; m < 3; m++) a.c1[ax][m] = (T)(W1[m] / h[ax]);
+    for (int i = 0; i < 3; i++) a.bext[i] = (T)ctx->bext[i];
+    for (int q = 0; q < AC_NFIELDS; q++) a.in[q] = (const T*)ctx->field_ptr(ctx->cur, q);
+    a.partial = (ac::RedVals*)(ctx->ws + ctx->cv.partial_off);
+    ac::RedVals* result = (ac::RedVals*)(ctx->ws + ctx->cv.result_off);
+    const long rows = (long)L.ny * L.nz;
+    const int blocks = (int)std::min<long>(rows, RED_BLOCKS);
+    ac::reduce_stage1_kernel<T><<<blocks, 256, 0, ctx->stream>>>(a);
+    ac::reduce_stage2_kernel<<<1, 256, 0, ctx->stream>>>(a.partial, blocks, result);
+    ctx->launches += 2;
+    AC_CUDA(cudaGetLastError());
+    AC_CUDA(cudaMemcpyAsync(ctx->host_result, result, sizeof(ac::RedVals), cudaMemcpyDeviceToHost, ctx->stream));
+    AC_CUDA(cudaStreamSynchronize(ctx->stream));
+    const ac::RedVals& r = *ctx->host_result;
+    const double ncell = (double)L.nx * L.ny * L.nz;
+    out->urms = std::sqrt(r.su / ncell);
+    out->umax = std::sqrt(r.mu);
+    out->brms = std::sqrt(r.sb / ncell);
+    out->bmax = std::sqrt(r.mb);
+    out->lnrho_min = r.lmin;
+    out->lnrho_max = r.lmax;
+    out->nonfinite = !(std::isfinite(r.su) && std::isfinite(r.sb) && std::isfinite(r.lmin) && std::isfinite(r.lmax));
+    const double hmin = std::min(h[0], std::min(h[1], h[2]));
+    double dt = ctx->c_u * hmin / (out->umax + ctx->cs);
+    const double d = std::max(ctx->nu, ctx->eta);
+    if (d > 0.0) dt = std::min(dt, ctx->c_nu * hmin * hmin / d);
+    out->dt_cfl = dt;
+    return AC_OK;
+}
+
+// ----- Eq. 4-6 on the host -----------------------------------------------------------------------
+void cross(const double a[3], const double b[3], double o[3]) {
+    o[0] = a[1] * b[2] - a[2] * b[1];
+    o[1] = a[2] * b[0] - a[0] * b[2];
+    o[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+uint64_t splitmix64(uint64_t x) {
+    x += 0x9E3779B97F4A7C15ull;
+    uint64_t z = x;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+
+std::vector<std::array<int, 3>>* build_shell(double k_f) {
+    auto* v = new (std::nothrow) std::vector<std::array<int, 3>>();
+    if (!v) return nullptr;
+    const double lo2 = (k_f - 0.5) * (k_f - 0.5), hi2 = (k_f + 0.5) * (k_f + 0.5);
+    const int r = (int)std::floor(k_f + 0.5);
+    // lexicographic order by construction (kx outermost)
+    for (int kx = -r; kx <= r; kx++)
+        for (int ky = -r; ky <= r; ky++)
+            for (int kz = -r; kz <= r; kz++) {
+                const double k2 = (double)kx * kx + (double)ky * ky + (double)kz * kz;
+                if (k2 >= lo2 && k2 <= hi2) v->push_back({kx, ky, kz});
+            }
+    return v;
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+size_t ac_workspace_bytes(const ac_grid* grid, ac_dtype dtype) {
+    if (!grid_ok(grid) || (dtype != AC_F32 && dtype != AC_F64)) return 0;
+    ac::Layout L = ac::make_layout(grid->nx, grid->ny, grid->nz, elem_size(dtype));
+    return carve(L, dtype).total;
+}
+
+int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double eta, double cs, double k_f,
+            double helicity, void* workspace_dev, void* cuda_stream) {
+    if (!out) return AC_EINVAL;
+    *out = nullptr;
+    if (!grid_ok(grid) || (dtype != AC_F32 && dtype != AC_F64)) return AC_EINVAL;
+    if (!(nu >= 0.0) || !(eta >= 0.0) || !(cs > 0.0) || !std::isfinite(nu) || !std::isfinite(eta) || !std::isfinite(cs))
+        return AC_EINVAL;
+    if (!(k_f >= 1.0) || !(k_f <= 64.0) || !(helicity >= 0.0) || !(helicity <= 1.0)) return AC_EINVAL;
+    if (workspace_dev && ((uintptr_t)workspace_dev % 256) != 0) return AC_EINVAL;
+
+    int dev = 0;
+    AC_CUDA(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    AC_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "device %s is sm_%d%d; this library is built for sm_100a only", prop.name,
+                 prop.major, prop.minor);
+        return AC_ECUDA;
+    }
+
+    ac_ctx* ctx = new (std::nothrow) ac_ctx();
+    if (!ctx) return AC_ENOMEM;
+    ctx->grid = *grid;
+    ctx->dtype = dtype;
+    ctx->nu = nu;
+    ctx->eta = eta;
+    ctx->cs = cs;
+    ctx->k_f = k_f;
+    ctx->helicity = helicity;
+    ctx->bext[0] = ctx->bext[1] = ctx->bext[2] = 0.0;
+    ctx->c_u = 0.4;
+    ctx->c_nu = 0.25;
+    ctx->variant = 0;
+    ctx->L = ac::make_layout(grid->nx, grid->ny, grid->nz, elem_size(dtype));
+    ctx->cv = carve(ctx->L, dtype);
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->cur = 0;
+    ctx->loaded = false;
+    ctx->launches = 0;
+    ctx->host_result = nullptr;
+    ctx->shell = nullptr;
+    if (workspace_dev) {
+        ctx->ws = (char*)workspace_dev;
+        ctx->owns_ws = false;
+    } else {
+        void* p = nullptr;
+        cudaError_t e = cudaMalloc(&p, ctx->cv.total);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            delete ctx->shell;
+            delete ctx;
+            return e == cudaErrorMemoryAllocation ? AC_ENOMEM : cuda_fail(e, "cudaMalloc(workspace)");
+        }
+        ctx->ws = (char*)p;
+        ctx->owns_ws = true;
+    }
+    cudaError_t e = cudaMallocHost((void**)&ctx->host_result, sizeof(ac::RedVals));
+    if (e != cudaSuccess) {
+        if (ctx->owns_ws) cudaFree(ctx->ws);
+        delete ctx->shell;
+        delete ctx;
+        return cuda_fail(e, "cudaMallocHost");
+    }
+    *out = ctx;
+    return AC_OK;
+}
+
+int ac_load_state(ac_ctx* ctx, const void* const fields[AC_NFIELDS], int src_on_device) {
+    if (!ctx || !fields) return AC_EINVAL;
+    for (int q = 0; q < AC_NFIELDS; q++)
+        if (!fields[q]) return AC_EINVAL;
+    return ctx->dtype == AC_F64 ? load_state_t<double>(ctx, fields, src_on_device)
+                                : load_state_t<float>(ctx, fields, src_on_device);
+}
+
+int ac_store_state(ac_ctx* ctx, void* const fields[AC_NFIELDS], int dst_on_device) {
+    if (!ctx || !fields) return AC_EINVAL;
+    for (int q = 0; q < AC_NFIELDS; q++)
+        if (!fields[q]) return AC_EINVAL;
+    if (!ctx->loaded) return AC_ESTATE;
+    return ctx->dtype == AC_F64 ? store_state_t<double>(ctx, fields, dst_on_device)
+                                : store_state_t<float>(ctx, fields, dst_on_device);
+}
+
+int ac_step(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
+    if (!ctx) return AC_EINVAL;
+    if (!(dt > 0.0) || !std::isfinite(dt)) return AC_EINVAL;
+    if (!ctx->loaded) return AC_ESTATE;
+    if (forcing) {
+        for (int i = 0; i < 3; i++)
+            if (!std::isfinite(forcing->k[i]) || !std::isfinite(forcing->re[i]) || !std::isfinite(forcing->im[i]))
+                return AC_EINVAL;
+        if (!std::isfinite(forcing->phase)) return AC_EINVAL;
+    }
+    return ctx->dtype == AC_F64 ? step_t<double>(ctx, dt, forcing) : step_t<float>(ctx, dt, forcing);
+}
+
+int ac_reduce(ac_ctx* ctx, ac_diag* out) {
+    if (!ctx || !out) return AC_EINVAL;
+    if (!ctx->loaded) return AC_ESTATE;
+    return ctx->dtype == AC_F64 ? reduce_t<double>(ctx, out) : reduce_t<float>(ctx, out);
+}
+
+int ac_forcing_params(double k_f, double helicity, double cs, const ac_grid* grid, double u1, double u2, double u3,
+                      double dt, double f0, ac_forcing* out) {
+    if (!out || !grid_ok(grid)) return AC_EINVAL;
+    if (!(k_f >= 1.0) || !(k_f <= 64.0) || !(helicity >= 0.0) || !(helicity <= 1.0) || !(cs > 0.0)) return AC_EINVAL;
+    if (!(u1 >= 0.0 && u1 < 1.0 && u2 >= 0.0 && u2 < 1.0 && u3 >= 0.0 && u3 < 1.0)) return AC_EINVAL;
+    if (!(dt > 0.0) || !std::isfinite(dt) || !std::isfinite(f0)) return AC_EINVAL;
+    std::vector<std::array<int, 3>>* shp = build_shell(k_f);
+    if (!shp) return AC_ENOMEM;
+    if (shp->empty()) {
+        delete shp;
+        return AC_EINVAL;
+    }
+    const auto& sh = *shp;
+    size_t idx = (size_t)std::floor(u1 * (double)sh.size());
+    if (idx >= sh.size()) idx = sh.size() - 1;
+    const double k[3] = {(double)sh[idx][0], (double)sh[idx][1], (double)sh[idx][2]};
+    delete shp;
+    const double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
+    const double kabs = std::sqrt(k2);
+    const double pi = 3.14159265358979323846;
+    // e-hat = cos(psi) e1 + sin(psi) e2, e1 = normalise(k x a), a = axis of smallest |k_a|, e2 = k^ x e1 (G9)
+    int ai = 0;
+    for (int i = 1; i < 3; i++)
+        if (std::fabs(k[i]) < std::fabs(k[ai])) ai = i;
+    double a[3] = {0, 0, 0};
+    a[ai] = 1.0;
+    double e1[3], e2[3], khat[3] = {k[0] / kabs, k[1] / kabs, k[2] / kabs};
+    cross(k, a, e1);
+    const double n1 = std::sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
+    for (int i = 0; i < 3; i++) e1[i] /= n1;
+    cross(khat, e1, e2);
+    const double psi = 2.0 * pi * u3;
+    double eh[3];
+    for (int i = 0; i < 3; i++) eh[i] = std::cos(psi) * e1[i] + std::sin(psi) * e2[i];
+    // Eq. 6: f_k = [k x (k x e) - i sigma |k| (k x e)] / [sqrt(1 + sigma^2) k^2 sqrt(1 - (k.e)^2/k^2)]
+    double kxe[3], kxkxe[3];
+    cross(k, eh, kxe);
+    cross(k, kxe, kxkxe);
+    const double sigma = helicity;
+    const double kde = k[0] * eh[0] + k[1] * eh[1] + k[2] * eh[2];
+    const double den = std::sqrt(1.0 + sigma * sigma) * k2 * std::sqrt(1.0 - kde * kde / k2);
+    // Eq. 5: N = f0 cs sqrt(|k| cs / dt)
+    const double N = f0 * cs * std::sqrt(kabs * cs / dt);
+    // the integer shell vector counts periods per box side: k_a 2 pi / l_a
+    out->k[0] = k[0] * (2.0 * pi / grid->lx);
+    out->k[1] = k[1] * (2.0 * pi / grid->ly);
+    out->k[2] = k[2] * (2.0 * pi / grid->lz);
+    out->phase = -pi + 2.0 * pi * u2;
+    for (int i = 0; i < 3; i++) {
+        out->re[i] = N * kxkxe[i] / den;
+        out->im[i] = N * (-sigma * kabs * kxe[i]) / den;
+    }
+    return AC_OK;
+}
+
+int ac_forcing_from_draws(const ac_ctx* ctx, double u1, double u2, double u3, double dt, double f0, ac_forcing* out) {
+    if (!ctx) return AC_EINVAL;
+    return ac_forcing_params(ctx->k_f, ctx->helicity, ctx->cs, &ctx->grid, u1, u2, u3, dt, f0, out);
+}
+
+int ac_make_forcing(const ac_ctx* ctx, uint64_t seed, uint64_t step, double dt, double f0, ac_forcing* out) {
+    if (!ctx || !out) return AC_EINVAL;
+    const uint64_t key = splitmix64(seed);
+    double u[3];
+    for (uint64_t i = 0; i < 3; i++) u[i] = (double)(splitmix64(key ^ (3 * step + i)) >> 11) * (1.0 / 9007199254740992.0);
+    return ac_forcing_from_draws(ctx, u[0], u[1], u[2], dt, f0, out);
+}
+
+int ac_set_bext(ac_ctx* ctx, const double b[3]) {
+    if (!ctx || !b) return AC_EINVAL;
+    for (int i = 0; i < 3; i++) {
+        if (!std::isfinite(b[i])) return AC_EINVAL;
+        ctx->bext[i] = b[i];
+    }
+    return AC_OK;
+}
+
+int ac_set_cfl(ac_ctx* ctx, double c_u, double c_nu) {
+    if (!ctx || !(c_u > 0.0) || !(c_nu > 0.0)) return AC_EINVAL;
+    ctx->c_u = c_u;
+    ctx->c_nu = c_nu;
+    return AC_OK;
+}
+
+int ac_set_variant(ac_ctx* ctx, int variant) {
+    if (!ctx) return AC_EINVAL;
+    if (variant != 0 && variant != 1) return AC_EINVAL;
+    ctx->variant = variant;
+    return AC_OK;
+}
+
+long long ac_launch_count(const ac_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+void ac_free(ac_ctx* ctx) {
+    if (!ctx) return;
+    cudaStreamSynchronize(ctx->stream);
+    if (ctx->owns_ws) cudaFree(ctx->ws);
+    if (ctx->host_result) cudaFreeHost(ctx->host_result);
+    delete ctx->shell;
+    delete ctx;
+}
+
+const char* ac_strerror(int status) {
+    switch (status) {
+        case AC_OK: return "ok";
+        case AC_EINVAL: return "invalid argument";
+        case AC_ENOMEM: return "out of memory or workspace too small";
+        case AC_ECUDA: return g_cuda_err;
+        case AC_ESTATE: return "no state loaded (call ac_load_state first)";
+        default: return "unknown status";
+    }
+}
+
+const char* ac_version(void) { return "ac_mhd 0.1 sm_100a"; }
+
+}  // extern "C"

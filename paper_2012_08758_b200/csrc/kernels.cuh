@@ -1,0 +1,255 @@
+// CUDA kernels of the hot path: state pack/unpack, forcing tables, the fused RK substep
+// (variant "direct": one thread per cell, neighbours through the read-only global path) and the
+// two-stage reductions.  sm_100a only.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+#include "layout.cuh"
+#include "mhd_cell.cuh"
+
+namespace ac {
+
+// ------------------------------------------------------------------------------------------------
+// dense <-> padded copies (S1: periodic halo = "local boundary transfer")
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void pack_kernel(const T* __restrict__ dense, T* __restrict__ padded, Layout L) {
+    // one thread per padded element that matters: x in [-R, nx+R), y in [-R, ny+R), z in [-R, nz+R)
+    const int px = blockIdx.x * blockDim.x + threadIdx.x - R;
+    const int py = blockIdx.y * blockDim.y + threadIdx.y - R;
+    const int pz = blockIdx.z - R;
+    if (px >= L.nx + R || py >= L.ny + R) return;
+    int sx = px < 0 ? px + L.nx : (px >= L.nx ? px - L.nx : px);
+    int sy = py < 0 ? py + L.ny : (py >= L.ny ? py - L.ny : py);
+    int sz = pz < 0 ? pz + L.nz : (pz >= L.nz ? pz - L.nz : pz);
+    padded[L.idx(px, py, pz)] = dense[(size_t)sx + (size_t)L.nx * ((size_t)sy + (size_t)L.ny * (size_t)sz)];
+}
+
+template <typename T>
+__global__ void unpack_kernel(const T* __restrict__ padded, T* __restrict__ dense, Layout L) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= L.nx || y >= L.ny) return;
+    dense[(size_t)x + (size_t)L.nx * ((size_t)y + (size_t)L.ny * (size_t)z)] = padded[L.idx(x, y, z)];
+}
+
+// ------------------------------------------------------------------------------------------------
+// forcing tables (S7): cos/sin of k_a x_a per axis, phase folded into the z table.
+// layout: [cx(nx) sx(nx) cy(ny) sy(ny) cz(nz) sz(nz)]
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void forcing_tables_kernel(T* __restrict__ tab, int nx, int ny, int nz, double kx, double ky, double kz,
+                                      double hx, double hy, double hz, double phase) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nx + ny + nz) return;
+    double th;
+    T *pc, *ps;
+    if (i < nx) {
+        th = kx * (i * hx);
+        pc = tab + i;
+        ps = tab + nx + i;
+    } else if (i < nx + ny) {
+        int j = i - nx;
+        th = ky * (j * hy);
+        pc = tab + 2 * nx + j;
+        ps = tab + 2 * nx + ny + j;
+    } else {
+        int j = i - nx - ny;
+        th = kz * (j * hz) + phase;
+        pc = tab + 2 * nx + 2 * ny + j;
+        ps = tab + 2 * nx + 2 * ny + nz + j;
+    }
+    double s, c;
+    sincos(th, &s, &c);
+    *pc = (T)c;
+    *ps = (T)s;
+}
+
+template <typename T>
+__device__ __forceinline__ void forcing_phase(const T* __restrict__ tab, int nx, int ny, int nz, int x, int y, int z,
+                                              T& fc, T& fs) {
+    const T cx = __ldg(tab + x), sx = __ldg(tab + nx + x);
+    const T cy = __ldg(tab + 2 * nx + y), sy = __ldg(tab + 2 * nx + ny + y);
+    const T cz = __ldg(tab + 2 * nx + 2 * ny + z), sz = __ldg(tab + 2 * nx + 2 * ny + nz + z);
+    const T cxy = cx * cy - sx * sy, sxy = sx * cy + cx * sy;
+    fc = cxy * cz - sxy * sz;
+    fs = sxy * cz + cxy * sz;
+}
+
+// ------------------------------------------------------------------------------------------------
+// fused substep, common argument block
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+struct SubstepArgs {
+    const T* in[NFIELDS];
+    T* out[NFIELDS];
+    const T* ftab;
+    Layout L;
+    Coeffs<T> c;
+    Physics<T> p;
+};
+
+// write a new interior value and its periodic images in the ghost layers (S1 fused into S8)
+template <typename T>
+__device__ __forceinline__ void store_with_images(T* __restrict__ o, const Layout& L, int x, int y, int z, T v,
+                                                  bool edge) {
+    o[L.idx(x, y, z)] = v;
+    if (!edge) return;
+    int xs[2] = {x, x}, ys[2] = {y, y}, zs[2] = {z, z};
+    int cx = 1, cy = 1, cz = 1;
+    if (x < R) xs[cx++] = x + L.nx; else if (x >= L.nx - R) xs[cx++] = x - L.nx;
+    if (y < R) ys[cy++] = y + L.ny; else if (y >= L.ny - R) ys[cy++] = y - L.ny;
+    if (z < R) zs[cz++] = z + L.nz; else if (z >= L.nz - R) zs[cz++] = z - L.nz;
+    for (int k = 0; k < cz; k++)
+        for (int j = 0; j < cy; j++)
+            for (int i = 0; i < cx; i++)
+                if (i + j + k) o[L.idx(xs[i], ys[j], zs[k])] = v;
+}
+
+// Variant "direct": one thread per cell, every stencil point fetched through the read-only
+// global/L1 path from the ghost-padded arrays.  Simple and obviously right; kept as the
+// debugging / cross-check variant (ac_set_variant(ctx, 1)).
+template <typename T>
+__global__ void __launch_bounds__(256) substep_direct_kernel(const __grid_constant__ SubstepArgs<T> a) {
+    const Layout& L = a.L;
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z * blockDim.z + threadIdx.z;
+    if (x >= L.nx || y >= L.ny || z >= L.nz) return;
+    const size_t c0 = L.idx(x, y, z);
+    const long pitch = L.pitch;
+    const long plane = (long)L.plane;
+    auto fetch = [&](int q, int dx, int dy, int dz) -> T {
+        return __ldg(a.in[q] + (c0 + dx + dy * pitch + dz * plane));
+    };
+    T prev[NFIELDS];
+#pragma unroll
+    for (int q = 0; q < NFIELDS; q++) prev[q] = (a.p.substep != 0) ? a.out[q][c0] : T(0);
+    T fc = T(0), fs = T(0);
+    if (a.p.has_forcing) forcing_phase<T>(a.ftab, L.nx, L.ny, L.nz, x, y, z, fc, fs);
+    T res[NFIELDS];
+    substep_cell<T>(fetch, a.c, a.p, prev, fc, fs, res);
+    const bool edge = (x < R) | (x >= L.nx - R) | (y < R) | (y >= L.ny - R) | (z < R) | (z >= L.nz - R);
+#pragma unroll
+    for (int q = 0; q < NFIELDS; q++) store_with_images<T>(a.out[q], L, x, y, z, res[q], edge);
+}
+
+// ------------------------------------------------------------------------------------------------
+// reductions (S9): sum and max of |u|^2 and |B|^2, min/max of ln rho.  Two stages, fixed order.
+// ------------------------------------------------------------------------------------------------
+struct RedVals {
+    double su, mu, sb, mb, lmin, lmax;
+};
+
+__device__ __forceinline__ RedVals red_combine(const RedVals& a, const RedVals& b) {
+    RedVals r;
+    r.su = a.su + b.su;
+    r.sb = a.sb + b.sb;
+    r.mu = fmax(a.mu, b.mu);
+    r.mb = fmax(a.mb, b.mb);
+    r.lmin = fmin(a.lmin, b.lmin);
+    r.lmax = fmax(a.lmax, b.lmax);
+    return r;
+}
+
+__device__ __forceinline__ RedVals red_shfl_down(const RedVals& v, int d) {
+    RedVals r;
+    r.su = __shfl_down_sync(0xffffffffu, v.su, d);
+    r.mu = __shfl_down_sync(0xffffffffu, v.mu, d);
+    r.sb = __shfl_down_sync(0xffffffffu, v.sb, d);
+    r.mb = __shfl_down_sync(0xffffffffu, v.mb, d);
+    r.lmin = __shfl_down_sync(0xffffffffu, v.lmin, d);
+    r.lmax = __shfl_down_sync(0xffffffffu, v.lmax, d);
+    return r;
+}
+
+// NaN-propagating identity: fmax/fmin drop NaNs, so non-finite input is tracked through the sums
+__device__ __forceinline__ RedVals red_identity() {
+    RedVals r;
+    r.su = 0.0;
+    r.sb = 0.0;
+    r.mu = 0.0;
+    r.mb = 0.0;
+    r.lmin = INFINITY;
+    r.lmax = -INFINITY;
+    return r;
+}
+
+__device__ __forceinline__ RedVals block_reduce(RedVals v) {
+    __shared__ RedVals warp_part[32];
+    const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+    const int lane = tid & 31, wid = tid >> 5;
+    const int nwarps = (blockDim.x * blockDim.y * blockDim.z + 31) >> 5;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v = red_combine(v, red_shfl_down(v, d));
+    if (lane == 0) warp_part[wid] = v;
+    __syncthreads();
+    if (wid == 0) {
+        v = lane < nwarps ? warp_part[lane] : red_identity();
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) v = red_combine(v, red_shfl_down(v, d));
+    }
+    return v;  // valid in thread 0
+}
+
+template <typename T>
+struct ReduceArgs {
+    const T* in[NFIELDS];
+    Layout L;
+    T c1[3][3];
+    T bext[3];
+    RedVals* partial;
+};
+
+// stage 1: each block owns a fixed set of (y, z) rows; one partial per block
+template <typename T>
+__global__ void __launch_bounds__(256) reduce_stage1_kernel(const __grid_constant__ ReduceArgs<T> a) {
+    const Layout& L = a.L;
+    RedVals acc = red_identity();
+    const long pitch = L.pitch, plane = (long)L.plane;
+    const long rows = (long)L.ny * L.nz;
+    for (long row = blockIdx.x; row < rows; row += gridDim.x) {
+        const int y = (int)(row % L.ny), z = (int)(row / L.ny);
+        for (int x = threadIdx.x; x < L.nx; x += blockDim.x) {
+            const size_t c0 = L.idx(x, y, z);
+            const T ux = a.in[UX][c0], uy = a.in[UY][c0], uz = a.in[UZ][c0];
+            const T l = a.in[LNRHO][c0];
+            auto d = [&](int q, long stride, int axis) -> T {
+                const T* p = a.in[q] + c0;
+                T r = a.c1[axis][0] * (p[stride] - p[-stride]);
+                r = fma_<T>(a.c1[axis][1], p[2 * stride] - p[-2 * stride], r);
+                r = fma_<T>(a.c1[axis][2], p[3 * stride] - p[-3 * stride], r);
+                return r;
+            };
+            const T bx = d(AZ, pitch, 1) - d(AY, plane, 2) + a.bext[0];
+            const T by = d(AX, plane, 2) - d(AZ, 1, 0) + a.bext[1];
+            const T bz = d(AY, 1, 0) - d(AX, pitch, 1) + a.bext[2];
+            const double u2 = (double)ux * ux + (double)uy * uy + (double)uz * uz;
+            const double b2 = (double)bx * bx + (double)by * by + (double)bz * bz;
+            acc.su += u2;
+            acc.sb += b2;
+            acc.mu = fmax(acc.mu, u2);
+            acc.mb = fmax(acc.mb, b2);
+            acc.lmin = fmin(acc.lmin, (double)l);
+            acc.lmax = fmax(acc.lmax, (double)l);
+            // a non-finite ln rho or A would hide in fmin/fmax: fold it into the sums
+            const double chk = (double)l + (double)a.in[AX][c0] + (double)a.in[AY][c0] + (double)a.in[AZ][c0];
+            if (!isfinite(chk)) acc.su += chk;
+        }
+    }
+    acc = block_reduce(acc);
+    if (threadIdx.x == 0) a.partial[blockIdx.x] = acc;
+}
+
+// stage 2: one block folds the per-block partials in a fixed order
+__global__ void __launch_bounds__(256) reduce_stage2_kernel(const RedVals* __restrict__ partial, int n,
+                                                            RedVals* __restrict__ result) {
+    RedVals acc = red_identity();
+    for (int i = threadIdx.x; i < n; i += blockDim.x) acc = red_combine(acc, partial[i]);
+    acc = block_reduce(acc);
+    if (threadIdx.x == 0) *result = acc;
+}
+
+}  // namespace ac

@@ -1,0 +1,247 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on the
+same seeded inputs.  Tolerances are BASELINE.json's: fp64 <= 1e-12 after 1 step and <= 1e-9 after
+10 steps, fp32 <= 1e-5 after 1 step, in the group-scaled max norm of DESIGN.md reading G14."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import mhd_c
+from paper_2012_08758_b200 import binding, inputs
+import helpers
+from helpers import TWO_PI3
+
+pytestmark = pytest.mark.gpu
+
+VARIANTS = [0, 1]
+
+
+def make_ctx(shape, dtype=binding.AC_F64, lengths=TWO_PI3, variant=0, **kw):
+    ctx = binding.Context(shape, lengths, dtype, **kw)
+    ctx.ac_set_variant(variant)
+    return ctx
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config1_32cubed_fp64_1_and_10_steps(variant):
+    seed, n, dt = 1001, 32, 1e-3
+    state = inputs.gaussian_state(n, seed)
+    ctx = make_ctx((n, n, n), nu=5e-3, eta=5e-3, cs=1.0, k_f=3, helicity=0.0, variant=variant)
+    ctx.ac_load_state(state)
+    assert np.array_equal(ctx.ac_store_state(), state)              # load/store round trip is exact
+    ff = lambda s: helpers.oracle_forcing(seed + 7, s, 3, 0.0, dt, 0.02, 1.0)
+    want = helpers.oracle_run(state, 10, dt, TWO_PI3, 5e-3, 5e-3, 1.0, ff)
+    for s in range(10):
+        f = ctx.ac_make_forcing(seed + 7, s, dt, 0.02)
+        ctx.ac_step(dt, f)
+        if s == 0:
+            err1 = helpers.group_errors(ctx.ac_store_state(), want[0])
+    err10 = helpers.group_errors(ctx.ac_store_state(), want[9])
+    print("config1 variant", variant, "1 step", err1, "10 steps", err10)
+    assert max(err1.values()) <= 1e-12
+    assert max(err10.values()) <= 1e-9
+    ctx.ac_free()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("sigma", [0.0, 0.5, 1.0])
+def test_noncubic_strong_field_all_terms(variant, sigma):
+    shape = (64, 48, 32)                                # nz, ny, nx; different spacing per axis
+    lengths = (2 * math.pi, 2 * math.pi, 2 * math.pi)
+    state = inputs.smooth_strong_state(shape, 77)
+    dt, nu, eta, cs = 2e-3, 3e-3, 4e-3, 1.1
+    ctx = make_ctx(shape, lengths=lengths, nu=nu, eta=eta, cs=cs, k_f=3, helicity=sigma, variant=variant)
+    ctx.ac_load_state(state)
+    ff = lambda s: helpers.oracle_forcing(5, s, 3, sigma, dt, 0.02, cs, lengths)
+    want = helpers.oracle_run(state, 2, dt, lengths, nu, eta, cs, ff)
+    for s in range(2):
+        ctx.ac_step(dt, ctx.ac_make_forcing(5, s, dt, 0.02))
+    err = helpers.group_errors(ctx.ac_store_state(), want[1], cs)
+    print("noncubic sigma", sigma, err)
+    assert max(err.values()) <= 2e-12
+    ctx.ac_free()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_inviscid_ideal_and_external_field(variant):
+    shape = (24, 20, 16)
+    state = inputs.smooth_strong_state(shape, 9)
+    dt = 1e-3
+    for nu, eta, bext in ((0.0, 0.0, (0.0, 0.0, 0.0)), (1e-2, 0.0, (0.3, -0.1, 0.2))):
+        ctx = make_ctx(shape, nu=nu, eta=eta, variant=variant)
+        ctx.ac_set_bext(bext)
+        ctx.ac_load_state(state)
+        ctx.ac_step(dt, None)
+        want = helpers.oracle_run(state, 1, dt, TWO_PI3, nu, eta, 1.0, None, bext)[0]
+        assert helpers.max_group_error(ctx.ac_store_state(), want) <= 1e-12
+        d = ctx.ac_reduce()
+        dw = mhd_c.diagnostics(want, TWO_PI3, bext)
+        for key in ("urms", "umax", "brms", "bmax", "lnrho_min", "lnrho_max"):
+            assert abs(d[key] - dw[key]) <= 1e-12 * max(abs(dw[key]), 1e-30), key
+        ctx.ac_free()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_fp32_one_step(variant):
+    n = 48
+    state64 = inputs.solenoidal_state(n, 1003)
+    state32 = state64.astype(np.float32)
+    dt, nu = 5e-3, 1e-3
+    ctx = make_ctx((n, n, n), dtype=binding.AC_F32, nu=nu, eta=nu, k_f=3, helicity=0.0, variant=variant)
+    ctx.ac_load_state(state32)
+    f = ctx.ac_make_forcing(1010, 0, dt, 0.02)
+    ctx.ac_step(dt, f)
+    got = ctx.ac_store_state()
+    assert got.dtype == np.float32
+    # the oracle starts from the fp32-rounded inputs (reading G14)
+    want = helpers.oracle_run(state32.astype(np.float64), 1, dt, TWO_PI3, nu, nu, 1.0,
+                              lambda s: helpers.oracle_forcing(1010, s, 3, 0.0, dt, 0.02, 1.0))[0]
+    err = helpers.group_errors(got, want)
+    print("fp32 one step", err)
+    assert max(err.values()) <= 1e-5
+    ctx.ac_free()
+
+
+def test_config2_cfl_loop_and_reductions_fp64():
+    """BASELINE config 2 scaled to what the oracle finishes in seconds: 64^3, helical forcing,
+    CFL dt from ac_reduce every step; diagnostics within 1e-12 of the oracle's."""
+    n, seed, nu = 64, 1002, 2e-3
+    state = inputs.gaussian_state(n, seed)
+    ctx = make_ctx((n, n, n), nu=nu, eta=nu, k_f=3, helicity=1.0)
+    ctx.ac_load_state(state)
+    st = mhd_c.Stepper(state, TWO_PI3, nu, nu, 1.0)
+    for s in range(4):
+        d = ctx.ac_reduce()
+        dw = st.diagnostics()
+        for key in ("urms", "umax", "brms", "bmax"):
+            assert abs(d[key] - dw[key]) <= 1e-12 * dw[key], (s, key, d[key], dw[key])
+        h = 2 * math.pi / n
+        dt_want = min(0.4 * h / (dw["umax"] + 1.0), 0.25 * h * h / nu)
+        assert abs(d["dt_cfl"] - dt_want) <= 1e-12 * dt_want and d["nonfinite"] == 0
+        dt = d["dt_cfl"]
+        ctx.ac_step(dt, ctx.ac_make_forcing(seed + 7, s, dt, 0.02))
+        st.step(dt, helpers.oracle_forcing(seed + 7, s, 3, 1.0, dt, 0.02, 1.0))
+    assert helpers.max_group_error(ctx.ac_store_state(), st.state) <= 1e-11
+    ctx.ac_free()
+
+
+@pytest.mark.parametrize("dtype", [binding.AC_F64, binding.AC_F32])
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_p14_translation_invariance_is_bitwise(dtype, variant):
+    """Roll every input by (sz, sy, sx) cells, step, roll back: bitwise equal, because the per-cell
+    arithmetic does not depend on position.  Catches tile seams, halo wrap and races."""
+    shape = (40, 36, 64)
+    npdt = np.float64 if dtype == binding.AC_F64 else np.float32
+    state = inputs.smooth_strong_state(shape, 21).astype(npdt)
+    ctx = make_ctx(shape, dtype=dtype, nu=2e-3, eta=3e-3, variant=variant)
+    outs = []
+    for shift in ((0, 0, 0), (7, 5, 13), (-3, 17, 31)):
+        rolled = np.ascontiguousarray(np.roll(state, shift, axis=(1, 2, 3)))
+        ctx.ac_load_state(rolled)
+        for _ in range(2):
+            ctx.ac_step(1e-3, None)
+        outs.append(np.roll(ctx.ac_store_state(), tuple(-s for s in shift), axis=(1, 2, 3)))
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+    ctx.ac_free()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_ragged_and_minimum_grids(variant):
+    for shape in ((8, 8, 8), (12, 20, 36), (9, 11, 44)):
+        state = inputs.gaussian_state(shape, 4, u_amp=1e-2, a_amp=1e-3)
+        state[0] = 0.1 * inputs.uniform_state(shape, 5)[0]
+        ctx = make_ctx(shape, nu=1e-2, eta=1e-2, helicity=1.0, variant=variant)
+        ctx.ac_load_state(state)
+        dt = 1e-3
+        f = ctx.ac_make_forcing(3, 0, dt, 0.02)
+        ctx.ac_step(dt, f)
+        want = helpers.oracle_run(state, 1, dt, TWO_PI3, 1e-2, 1e-2, 1.0,
+                                  lambda s: helpers.oracle_forcing(3, s, 3, 1.0, dt, 0.02, 1.0))[0]
+        assert helpers.max_group_error(ctx.ac_store_state(), want) <= 1e-12, shape
+        ctx.ac_free()
+
+
+def test_variants_agree_and_run_to_run_determinism():
+    shape = (32, 32, 64)
+    state = inputs.smooth_strong_state(shape, 31)
+    res = []
+    for variant in VARIANTS + VARIANTS[:1]:
+        ctx = make_ctx(shape, nu=1e-3, eta=1e-3, variant=variant)
+        ctx.ac_load_state(state)
+        for s in range(3):
+            ctx.ac_step(1e-3, ctx.ac_make_forcing(1, s, 1e-3, 0.02))
+        res.append((ctx.ac_store_state(), ctx.ac_reduce()))
+        ctx.ac_free()
+    assert np.array_equal(res[0][0], res[-1][0]) and res[0][1] == res[-1][1]       # same variant twice: bitwise
+    assert helpers.max_group_error(res[1][0], res[0][0]) <= 1e-13
+
+
+def test_state_errors_and_device_buffers():
+    import torch
+    shape = (16, 16, 16)
+    ctx = make_ctx(shape, nu=1e-3, eta=1e-3)
+    with pytest.raises(binding.AcError):
+        ctx.ac_step(1e-3, None)                       # AC_ESTATE: nothing loaded
+    with pytest.raises(binding.AcError):
+        ctx.ac_reduce()
+    state = inputs.gaussian_state(shape, 2)
+    dev = torch.from_numpy(state).cuda()
+    ctx.ac_load_state(dev)                            # device source
+    with pytest.raises(binding.AcError):
+        ctx.ac_step(0.0, None)                        # AC_EINVAL
+    with pytest.raises(binding.AcError):
+        ctx.ac_step(float("nan"), None)
+    out = torch.empty_like(dev)
+    ctx.ac_store_state(out)                           # device destination
+    ctx.synchronize()
+    assert torch.equal(out, dev)
+    n0 = ctx.ac_launch_count()
+    ctx.ac_step(1e-3, None)
+    assert ctx.ac_launch_count() - n0 == 3            # exactly three fused substep kernels
+    ctx.ac_step(1e-3, ctx.ac_make_forcing(1, 0, 1e-3, 0.02))
+    assert ctx.ac_launch_count() - n0 == 7            # + forcing table kernel
+    # a NaN in the state is reported
+    bad = state.copy()
+    bad[5, 3, 3, 3] = np.nan
+    ctx.ac_load_state(bad)
+    assert ctx.ac_reduce()["nonfinite"] == 1
+    ctx.ac_free()
+
+
+@pytest.mark.parametrize("dtype,n", [(binding.AC_F64, 256), (binding.AC_F32, 256), (binding.AC_F64, 512),
+                                     (binding.AC_F32, 512)])
+def test_sampled_parity_at_baseline_sizes(dtype, n):
+    """BASELINE configs 3 (256^3) and 4 (512^3), in the launch configuration bench.py times:
+    one step, checked at sampled cells (corners, faces, interior) that the oracle computes one
+    by one on 24^3 periodic-extracted sub-boxes."""
+    npdt = np.float64 if dtype == binding.AC_F64 else np.float32
+    cfg = {256: dict(seed=1003, nu=1e-3, sigma=0.0), 512: dict(seed=1004, nu=5e-4, sigma=1.0)}[n]
+    state = inputs.solenoidal_state(n, cfg["seed"]).astype(npdt)
+    ctx = make_ctx((n, n, n), dtype=dtype, nu=cfg["nu"], eta=cfg["nu"], k_f=3, helicity=cfg["sigma"])
+    ctx.ac_load_state(state)
+    # dt and forcing for the oracle come from the oracle side, never from the CUDA path
+    h = 2 * math.pi / n
+    umax = float(np.sqrt((state[1:4].astype(np.float64) ** 2).sum(axis=0).max()))
+    dt = min(0.4 * h / (umax + 1.0), 0.25 * h * h / cfg["nu"])
+    d = ctx.ac_reduce()
+    assert abs(d["dt_cfl"] - dt) <= (1e-12 if dtype == binding.AC_F64 else 1e-6) * dt
+    assert abs(d["urms"] - 0.1) < 1e-6
+    f_oracle = helpers.oracle_forcing(cfg["seed"] + 7, 0, 3, cfg["sigma"], dt, 0.02, 1.0)
+    ctx.ac_step(dt, ctx.ac_make_forcing(cfg["seed"] + 7, 0, dt, 0.02))
+    got = ctx.ac_store_state()
+    ctx.ac_free()
+    rng = np.random.default_rng(n)
+    cells = [(0, 0, 0), (n - 1, n - 1, n - 1), (0, n - 1, 5), (n // 2, 0, n - 2), (3, n - 3, n // 2)]
+    cells += [tuple(int(v) for v in rng.integers(0, n, 3)) for _ in range(7)]
+    s_u = float(np.abs(state[1:4]).max())
+    s_a = float(np.abs(state[4:7]).max())
+    scale = np.array([s_u, s_u, s_u, s_u, s_a, s_a, s_a])
+    tol = 1e-12 if dtype == binding.AC_F64 else 1e-5
+    worst = 0.0
+    state64 = state.astype(np.float64) if dtype == binding.AC_F32 else state
+    for c in cells:
+        want = helpers.subbox_oracle_step(state64, c, dt, TWO_PI3, cfg["nu"], cfg["nu"], 1.0, f_oracle)
+        err = np.abs(got[:, c[0], c[1], c[2]].astype(np.float64) - want) / scale
+        worst = max(worst, float(err.max()))
+    print("sampled parity", n, npdt.__name__, worst)
+    assert worst <= tol
