@@ -2,19 +2,23 @@
 // launches, the Eq. 4-6 host helpers.  No torch, no exceptions across the boundary.
 #include "../../include/ac_mhd.h"
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
 #include <array>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
+#include <type_traits>
 #include <vector>
 
 #include "kernels.cuh"
 #include "layout.cuh"
 #include "mhd_cell.cuh"
+#include "substep_ring.cuh"
 
 namespace {
 
@@ -72,6 +76,47 @@ Carve carve(const ac::Layout& L, ac_dtype d) {
     return c;
 }
 
+// ring-kernel tile configurations: fp64 16x16 tiles, fp32 32x16 tiles, 8 plane slots
+using RingF64 = ac::RingCfg<double, 16, 16, 8, 3>;
+using RingF32 = ac::RingCfg<float, 32, 16, 8, 4>;
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// 4-D map (x, y, z, field) over one ghost-padded state buffer; box = (wx, wy, 1, 7)
+int make_state_map(CUtensorMap* map, void* base, const ac::Layout& L, size_t es, int wx, int wy) {
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled not available from the driver");
+        return AC_ECUDA;
+    }
+    cuuint64_t dims[4] = {(cuuint64_t)L.pitch, (cuuint64_t)L.my, (cuuint64_t)L.mz, (cuuint64_t)AC_NFIELDS};
+    cuuint64_t strides[3] = {(cuuint64_t)L.pitch * es, (cuuint64_t)L.plane * es, (cuuint64_t)L.field * es};
+    cuuint32_t box[4] = {(cuuint32_t)wx, (cuuint32_t)wy, 1u, (cuuint32_t)AC_NFIELDS};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = enc(map, es == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims,
+                     strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+        return AC_ECUDA;
+    }
+    return AC_OK;
+}
+
 }  // namespace
 
 struct ac_ctx {
@@ -91,6 +136,8 @@ struct ac_ctx {
     long long launches;
     ac::RedVals* host_result;  // pinned
     std::vector<std::array<int, 3>>* shell;
+    CUtensorMap map[2];  // TMA maps of the two state buffers (ring kernel)
+    int cz;              // planes per z chunk of the ring kernel
 
     void* field_ptr(int buf, int q) const { return ws + ((size_t)buf * AC_NFIELDS + q) * cv.field_bytes; }
 };
@@ -191,10 +238,15 @@ int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
             a.in[q] = (const T*)ctx->field_ptr(ctx->cur, q);
             a.out[q] = (T*)ctx->field_ptr(1 - ctx->cur, q);
         }
-        {
+        if (ctx->variant == 1) {
             dim3 blk(32, 4, 2);
             dim3 grd((L.nx + blk.x - 1) / blk.x, (L.ny + blk.y - 1) / blk.y, (L.nz + blk.z - 1) / blk.z);
             ac::substep_direct_kernel<T><<<grd, blk, 0, ctx->stream>>>(a);
+        } else {
+            using Cfg = typename std::conditional<sizeof(T) == 8, RingF64, RingF32>::type;
+            dim3 blk(Cfg::TX, Cfg::TY, 1);
+            dim3 grd((L.nx + Cfg::TX - 1) / Cfg::TX, (L.ny + Cfg::TY - 1) / Cfg::TY, (L.nz + ctx->cz - 1) / ctx->cz);
+            ac::substep_ring_kernel<T, Cfg><<<grd, blk, Cfg::SMEM_BYTES, ctx->stream>>>(a, ctx->map[ctx->cur], ctx->cz);
         }
         ctx->launches++;
         ctx->cur = 1 - ctx->cur;
@@ -336,6 +388,28 @@ int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double
         }
         ctx->ws = (char*)p;
         ctx->owns_ws = true;
+    }
+    {
+        int rc;
+        const size_t es = elem_size(dtype);
+        const int wx = dtype == AC_F64 ? RingF64::WX : RingF32::WX, wy = dtype == AC_F64 ? RingF64::WY : RingF32::WY;
+        rc = make_state_map(&ctx->map[0], ctx->field_ptr(0, 0), ctx->L, es, wx, wy);
+        if (rc == AC_OK) rc = make_state_map(&ctx->map[1], ctx->field_ptr(1, 0), ctx->L, es, wx, wy);
+        cudaError_t ea = dtype == AC_F64
+                             ? cudaFuncSetAttribute(ac::substep_ring_kernel<double, RingF64>,
+                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, RingF64::SMEM_BYTES)
+                             : cudaFuncSetAttribute(ac::substep_ring_kernel<float, RingF32>,
+                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, RingF32::SMEM_BYTES);
+        if (rc == AC_OK && ea != cudaSuccess) rc = cuda_fail(ea, "cudaFuncSetAttribute(ring kernel smem)");
+        if (rc != AC_OK) {
+            if (ctx->owns_ws) cudaFree(ctx->ws);
+            delete ctx->shell;
+            delete ctx;
+            return rc;
+        }
+        // z chunk: long enough to amortise the 6 halo planes, short enough for >= ~8 waves of CTAs
+        ctx->cz = 64;
+        if (const char* e = getenv("AC_RING_CZ")) ctx->cz = std::max(1, atoi(e));
     }
     cudaError_t e = cudaMallocHost((void**)&ctx->host_result, sizeof(ac::RedVals));
     if (e != cudaSuccess) {
