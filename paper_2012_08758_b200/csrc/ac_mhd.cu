@@ -77,7 +77,7 @@ Carve carve(const ac::Layout& L, ac_dtype d) {
 }
 
 // ring-kernel tile configurations: fp64 16x16 tiles, fp32 32x16 tiles, 8 plane slots
-using RingF64 = ac::RingCfg<double, 16, 16, 8, 3>;
+using RingF64 = ac::RingCfg<double, 16, 12, 8, 4>;
 using RingF32 = ac::RingCfg<float, 32, 16, 8, 4>;
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
