@@ -18,7 +18,8 @@
 #include "kernels.cuh"
 #include "layout.cuh"
 #include "mhd_cell.cuh"
-#include "substep_ring.cuh"
+#include "substep_march.cuh"
+#include "vec2.cuh"
 
 namespace {
 
@@ -62,12 +63,14 @@ struct Carve {
     size_t field_bytes, ftab_off, partial_off, result_off, total;
 };
 
-Carve carve(const ac::Layout& L, ac_dtype d) {
+// es = bytes per storage element (8: fp64 cells or packed fp32 pairs; 4: plain fp32 cells);
+// es_tab = bytes per forcing-table entry (the context's dtype)
+Carve carve(const ac::Layout& L, size_t es, size_t es_tab, int nz_full) {
     Carve c;
-    c.field_bytes = L.field * elem_size(d);
+    c.field_bytes = L.field * es;
     size_t off = 2 * AC_NFIELDS * c.field_bytes;
     c.ftab_off = off;
-    off += align_up((size_t)2 * (L.nx + L.ny + L.nz) * elem_size(d), 256);
+    off += align_up((size_t)2 * (L.nx + L.ny + nz_full) * es_tab, 256);
     c.partial_off = off;
     off += align_up(sizeof(ac::RedVals) * RED_BLOCKS, 256);
     c.result_off = off;
@@ -76,9 +79,16 @@ Carve carve(const ac::Layout& L, ac_dtype d) {
     return c;
 }
 
-// ring-kernel tile configurations: fp64 16x16 tiles, fp32 32x16 tiles, 8 plane slots
-using RingF64 = ac::RingCfg<double, 16, 12, 8, 4>;
-using RingF32 = ac::RingCfg<float, 32, 16, 8, 4>;
+// The two device layouts a context can use:
+//   march  - 8-byte elements: fp64 cells, or fp32 cells packed in (z, z + nz/2) pairs (needs nz even)
+//   plain  - fp32 cells, 4-byte elements (direct variant, or odd nz)
+bool can_pack(const ac_grid* g) { return g->nz % 2 == 0; }
+ac::Layout layout_for(const ac_grid* g, ac_dtype d, bool packed) {
+    if (d == AC_F64) return ac::make_layout(g->nx, g->ny, g->nz, 8);
+    if (packed) return ac::make_layout(g->nx, g->ny, g->nz / 2, 8);
+    return ac::make_layout(g->nx, g->ny, g->nz, 4);
+}
+size_t store_elem_size(ac_dtype d, bool packed) { return (d == AC_F64 || packed) ? 8 : 4; }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -96,20 +106,22 @@ EncodeTiledFn get_encode_fn() {
     return fn;
 }
 
-// 4-D map (x, y, z, field) over one ghost-padded state buffer; box = (wx, wy, 1, 7)
-int make_state_map(CUtensorMap* map, void* base, const ac::Layout& L, size_t es, int wx, int wy) {
+// 4-D map (x, y, z, field) over one ghost-padded state buffer of 8-byte elements; box = (wx, wy, 1, 7).
+// Boxes must start 16-byte aligned in global memory (an 8-byte-aligned start faults on B200).
+int make_state_map(CUtensorMap* map, void* base, const ac::Layout& L, int wx, int wy) {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) {
         snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled not available from the driver");
         return AC_ECUDA;
     }
+    const size_t es = 8;
     cuuint64_t dims[4] = {(cuuint64_t)L.pitch, (cuuint64_t)L.my, (cuuint64_t)L.mz, (cuuint64_t)AC_NFIELDS};
     cuuint64_t strides[3] = {(cuuint64_t)L.pitch * es, (cuuint64_t)L.plane * es, (cuuint64_t)L.field * es};
     cuuint32_t box[4] = {(cuuint32_t)wx, (cuuint32_t)wy, 1u, (cuuint32_t)AC_NFIELDS};
     cuuint32_t estr[4] = {1, 1, 1, 1};
-    CUresult r = enc(map, es == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims,
-                     strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                     CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
         return AC_ECUDA;
@@ -125,8 +137,10 @@ struct ac_ctx {
     double nu, eta, cs, k_f, helicity;
     double bext[3];
     double c_u, c_nu;
-    int variant;
-    ac::Layout L;
+    int variant;         // requested: 0 = scatter-march, 1 = direct
+    bool march;          // the kernel actually used (fp32 with odd nz falls back to direct)
+    bool packed;         // fp32 cells stored as (z, z + nz/2) pairs
+    ac::Layout L;        // layout in storage elements
     Carve cv;
     char* ws;
     bool owns_ws;
@@ -135,9 +149,9 @@ struct ac_ctx {
     bool loaded;
     long long launches;
     ac::RedVals* host_result;  // pinned
-    std::vector<std::array<int, 3>>* shell;
-    CUtensorMap map[2];  // TMA maps of the two state buffers (ring kernel)
-    int cz;              // planes per z chunk of the ring kernel
+    CUtensorMap map_in[2];     // TMA maps of the two state buffers: tile + halo boxes
+    CUtensorMap map_prev[2];   // and interior-tile boxes (previous state of the 2N update)
+    int cz, nchunks;           // z chunking of the march kernel
 
     void* field_ptr(int buf, int q) const { return ws + ((size_t)buf * AC_NFIELDS + q) * cv.field_bytes; }
 };
@@ -162,11 +176,11 @@ void fill_coeffs(const ac_ctx* ctx, ac::Coeffs<T>& c) {
 template <typename T>
 int load_state_t(ac_ctx* ctx, const void* const fields[AC_NFIELDS], int src_on_device) {
     const ac::Layout& L = ctx->L;
-    const size_t dense_bytes = (size_t)L.nx * L.ny * L.nz * sizeof(T);
+    const ac_grid& g = ctx->grid;
+    const size_t dense_bytes = (size_t)g.nx * g.ny * g.nz * sizeof(T);
     dim3 blk(64, 4, 1);
     dim3 grd((L.nx + 2 * ac::R + blk.x - 1) / blk.x, (L.ny + 2 * ac::R + blk.y - 1) / blk.y, L.nz + 2 * ac::R);
     for (int q = 0; q < AC_NFIELDS; q++) {
-        T* dst = (T*)ctx->field_ptr(0, q);
         const T* src;
         if (src_on_device) {
             src = (const T*)fields[q];
@@ -176,7 +190,10 @@ int load_state_t(ac_ctx* ctx, const void* const fields[AC_NFIELDS], int src_on_d
             AC_CUDA(cudaMemcpyAsync(stage, fields[q], dense_bytes, cudaMemcpyHostToDevice, ctx->stream));
             src = stage;
         }
-        ac::pack_kernel<T><<<grd, blk, 0, ctx->stream>>>(src, dst, L);
+        if (ctx->packed)
+            ac::pack_pairs_kernel<<<grd, blk, 0, ctx->stream>>>((const float*)src, (float2*)ctx->field_ptr(0, q), L, g.nz);
+        else
+            ac::pack_kernel<T><<<grd, blk, 0, ctx->stream>>>(src, (T*)ctx->field_ptr(0, q), L);
         ctx->launches++;
     }
     AC_CUDA(cudaGetLastError());
@@ -188,18 +205,17 @@ int load_state_t(ac_ctx* ctx, const void* const fields[AC_NFIELDS], int src_on_d
 template <typename T>
 int store_state_t(ac_ctx* ctx, void* const fields[AC_NFIELDS], int dst_on_device) {
     const ac::Layout& L = ctx->L;
-    const size_t dense_bytes = (size_t)L.nx * L.ny * L.nz * sizeof(T);
+    const ac_grid& g = ctx->grid;
+    const size_t dense_bytes = (size_t)g.nx * g.ny * g.nz * sizeof(T);
     dim3 blk(64, 4, 1);
     dim3 grd((L.nx + blk.x - 1) / blk.x, (L.ny + blk.y - 1) / blk.y, L.nz);
     for (int q = 0; q < AC_NFIELDS; q++) {
-        const T* src = (const T*)ctx->field_ptr(ctx->cur, q);
-        if (dst_on_device) {
-            ac::unpack_kernel<T><<<grd, blk, 0, ctx->stream>>>(src, (T*)fields[q], L);
-        } else {
-            T* stage = (T*)ctx->field_ptr(1 - ctx->cur, q);
-            ac::unpack_kernel<T><<<grd, blk, 0, ctx->stream>>>(src, stage, L);
-            AC_CUDA(cudaMemcpyAsync(fields[q], stage, dense_bytes, cudaMemcpyDeviceToHost, ctx->stream));
-        }
+        T* dst = dst_on_device ? (T*)fields[q] : (T*)ctx->field_ptr(1 - ctx->cur, q);
+        if (ctx->packed)
+            ac::unpack_pairs_kernel<<<grd, blk, 0, ctx->stream>>>((const float2*)ctx->field_ptr(ctx->cur, q), (float*)dst, L);
+        else
+            ac::unpack_kernel<T><<<grd, blk, 0, ctx->stream>>>((const T*)ctx->field_ptr(ctx->cur, q), dst, L);
+        if (!dst_on_device) AC_CUDA(cudaMemcpyAsync(fields[q], dst, dense_bytes, cudaMemcpyDeviceToHost, ctx->stream));
         ctx->launches++;
     }
     AC_CUDA(cudaGetLastError());
@@ -207,49 +223,127 @@ int store_state_t(ac_ctx* ctx, void* const fields[AC_NFIELDS], int dst_on_device
     return AC_OK;
 }
 
+// weights of the scatter-march kernel (substep_march.cuh), computed in fp64 and rounded once
+template <typename E>
+void fill_march_coef(const ac_ctx* ctx, ac::MarchCoef<E>& c, double dt, int s, const ac_forcing* forcing) {
+    using S = ac::Splat<E>;
+    const double h[3] = {ctx->grid.lx / ctx->grid.nx, ctx->grid.ly / ctx->grid.ny, ctx->grid.lz / ctx->grid.nz};
+    double c1[3][3], c2[3][3], c20[3];
+    for (int a = 0; a < 3; a++) {
+        for (int m = 0; m < 3; m++) {
+            c1[a][m] = W1[m] / h[a];
+            c2[a][m] = W2[m] / (h[a] * h[a]);
+        }
+        c20[a] = W2_0 / (h[a] * h[a]);
+    }
+    for (int m = 0; m < 3; m++) {
+        c.c1x[m] = S::of(c1[0][m]);
+        c.c1y[m] = S::of(c1[1][m]);
+        c.c1z[m] = S::of(c1[2][m]);
+        c.nc1z[m] = S::of(-c1[2][m]);
+        const double mxy = WM[m] / (h[0] * h[1]), mxz = WM[m] / (h[0] * h[2]), myz = WM[m] / (h[1] * h[2]);
+        c.cm3xy[m] = S::of(mxy / 3.0);
+        c.cm3xz[m] = S::of(mxz / 3.0);
+        c.ncm3xz[m] = S::of(-mxz / 3.0);
+        c.cm3yz[m] = S::of(myz / 3.0);
+        c.ncm3yz[m] = S::of(-myz / 3.0);
+        c.cmxy[m] = S::of(mxy);
+        c.cmxz[m] = S::of(mxz);
+        c.ncmxz[m] = S::of(-mxz);
+        c.cmyz[m] = S::of(myz);
+        c.ncmyz[m] = S::of(-myz);
+        c.c2x[m] = S::of(c2[0][m]);
+        c.c2y[m] = S::of(c2[1][m]);
+        c.c2z[m] = S::of(c2[2][m]);
+        c.nc2x[m] = S::of(-c2[0][m]);
+        c.nc2y[m] = S::of(-c2[1][m]);
+        c.nc2z[m] = S::of(-c2[2][m]);
+    }
+    for (int i = 0; i < 3; i++) {
+        // L_i = lap u_i + 1/3 (grad div u)_i: the second derivative along axis i carries 4/3
+        const double fx = (i == 0) ? 4.0 / 3.0 : 1.0, fy = (i == 1) ? 4.0 / 3.0 : 1.0, fz = (i == 2) ? 4.0 / 3.0 : 1.0;
+        for (int m = 0; m < 3; m++) {
+            c.w2x[i][m] = S::of(fx * c2[0][m]);
+            c.w2y[i][m] = S::of(fy * c2[1][m]);
+            c.w2z[i][m] = S::of(fz * c2[2][m]);
+        }
+        c.w20[i] = S::of(fx * c20[0] + fy * c20[1] + fz * c20[2]);
+    }
+    c.c20all = S::of(c20[0] + c20[1] + c20[2]);
+    c.nc20yz = S::of(-(c20[1] + c20[2]));
+    c.nc20xz = S::of(-(c20[0] + c20[2]));
+    c.nc20xy = S::of(-(c20[0] + c20[1]));
+    c.nu = S::of(ctx->nu);
+    c.eta = S::of(ctx->eta);
+    c.ncs2 = S::of(-(ctx->cs * ctx->cs));
+    c.n23 = S::of(-2.0 / 3.0);
+    for (int i = 0; i < 3; i++) {
+        c.bext[i] = S::of(ctx->bext[i]);
+        c.fre[i] = S::of(forcing ? forcing->re[i] : 0.0);
+        c.nfim[i] = S::of(forcing ? -forcing->im[i] : 0.0);
+    }
+    c.rk_a = S::of(s == 0 ? 0.0 : RK_BETA[s] * RK_ALPHA[s] / RK_BETA[s - 1]);
+    c.rk_b = S::of(RK_BETA[s] * dt);
+}
+
 template <typename T>
 int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
     const ac::Layout& L = ctx->L;
-    ac::SubstepArgs<T> a;
-    a.L = L;
-    fill_coeffs<T>(ctx, a.c);
-    a.p.nu = (T)ctx->nu;
-    a.p.eta = (T)ctx->eta;
-    a.p.cs2 = (T)(ctx->cs * ctx->cs);
-    for (int i = 0; i < 3; i++) a.p.bext[i] = (T)ctx->bext[i];
-    a.p.has_forcing = forcing ? 1 : 0;
-    for (int i = 0; i < 3; i++) {
-        a.p.fre[i] = forcing ? (T)forcing->re[i] : T(0);
-        a.p.fim[i] = forcing ? (T)forcing->im[i] : T(0);
-    }
-    a.ftab = (const T*)(ctx->ws + ctx->cv.ftab_off);
+    const ac_grid& g = ctx->grid;
+    T* ftab = (T*)(ctx->ws + ctx->cv.ftab_off);
     if (forcing) {
-        const int n = L.nx + L.ny + L.nz;
+        const int n = g.nx + g.ny + g.nz;
         ac::forcing_tables_kernel<T><<<(n + 255) / 256, 256, 0, ctx->stream>>>(
-            (T*)(ctx->ws + ctx->cv.ftab_off), L.nx, L.ny, L.nz, forcing->k[0], forcing->k[1], forcing->k[2],
-            ctx->grid.lx / L.nx, ctx->grid.ly / L.ny, ctx->grid.lz / L.nz, forcing->phase);
+            ftab, g.nx, g.ny, g.nz, forcing->k[0], forcing->k[1], forcing->k[2], g.lx / g.nx, g.ly / g.ny, g.lz / g.nz,
+            forcing->phase);
         ctx->launches++;
     }
-    for (int s = 0; s < 3; s++) {
-        a.p.substep = s;
-        a.p.rk_a = (s == 0) ? T(0) : (T)(RK_BETA[s] * RK_ALPHA[s] / RK_BETA[s - 1]);
-        a.p.rk_b = (T)(RK_BETA[s] * dt);
-        for (int q = 0; q < AC_NFIELDS; q++) {
-            a.in[q] = (const T*)ctx->field_ptr(ctx->cur, q);
-            a.out[q] = (T*)ctx->field_ptr(1 - ctx->cur, q);
+    if (ctx->march) {
+        using E = typename ac::ElemOf<T>::E;
+        ac::MarchArgs<T> a;
+        a.ftab = ftab;
+        a.L = L;
+        a.nz_full = g.nz;
+        a.cz = ctx->cz;
+        a.has_forcing = forcing ? 1 : 0;
+        for (int s = 0; s < 3; s++) {
+            a.substep = s;
+            fill_march_coef<E>(ctx, a.c, dt, s, forcing);
+            for (int q = 0; q < AC_NFIELDS; q++) a.out[q] = (E*)ctx->field_ptr(1 - ctx->cur, q);
+            dim3 grd((L.nx + ac::M_TX - 1) / ac::M_TX, (L.ny + ac::M_TY - 1) / ac::M_TY, ctx->nchunks);
+            ac::substep_march_kernel<T><<<grd, ac::M_THREADS, ac::M_SMEM_BYTES, ctx->stream>>>(
+                a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
+            ctx->launches++;
+            ctx->cur = 1 - ctx->cur;
         }
-        if (ctx->variant == 1) {
+    } else {
+        ac::SubstepArgs<T> a;
+        a.L = L;
+        fill_coeffs<T>(ctx, a.c);
+        a.p.nu = (T)ctx->nu;
+        a.p.eta = (T)ctx->eta;
+        a.p.cs2 = (T)(ctx->cs * ctx->cs);
+        for (int i = 0; i < 3; i++) a.p.bext[i] = (T)ctx->bext[i];
+        a.p.has_forcing = forcing ? 1 : 0;
+        for (int i = 0; i < 3; i++) {
+            a.p.fre[i] = forcing ? (T)forcing->re[i] : T(0);
+            a.p.fim[i] = forcing ? (T)forcing->im[i] : T(0);
+        }
+        a.ftab = ftab;
+        for (int s = 0; s < 3; s++) {
+            a.p.substep = s;
+            a.p.rk_a = (s == 0) ? T(0) : (T)(RK_BETA[s] * RK_ALPHA[s] / RK_BETA[s - 1]);
+            a.p.rk_b = (T)(RK_BETA[s] * dt);
+            for (int q = 0; q < AC_NFIELDS; q++) {
+                a.in[q] = (const T*)ctx->field_ptr(ctx->cur, q);
+                a.out[q] = (T*)ctx->field_ptr(1 - ctx->cur, q);
+            }
             dim3 blk(32, 4, 2);
             dim3 grd((L.nx + blk.x - 1) / blk.x, (L.ny + blk.y - 1) / blk.y, (L.nz + blk.z - 1) / blk.z);
             ac::substep_direct_kernel<T><<<grd, blk, 0, ctx->stream>>>(a);
-        } else {
-            using Cfg = typename std::conditional<sizeof(T) == 8, RingF64, RingF32>::type;
-            dim3 blk(Cfg::TX, Cfg::TY, 1);
-            dim3 grd((L.nx + Cfg::TX - 1) / Cfg::TX, (L.ny + Cfg::TY - 1) / Cfg::TY, (L.nz + ctx->cz - 1) / ctx->cz);
-            ac::substep_ring_kernel<T, Cfg><<<grd, blk, Cfg::SMEM_BYTES, ctx->stream>>>(a, ctx->map[ctx->cur], ctx->cz);
+            ctx->launches++;
+            ctx->cur = 1 - ctx->cur;
         }
-        ctx->launches++;
-        ctx->cur = 1 - ctx->cur;
     }
     AC_CUDA(cudaGetLastError());
     return AC_OK;
@@ -258,25 +352,29 @@ int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
 template <typename T>
 int reduce_t(ac_ctx* ctx, ac_diag* out) {
     const ac::Layout& L = ctx->L;
+    const ac_grid& g = ctx->grid;
     ac::ReduceArgs<T> a;
     a.L = L;
-    const double h[3] = {ctx->grid.lx / L.nx, ctx->grid.ly / L.ny, ctx->grid.lz / L.nz};
+    const double h[3] = {g.lx / g.nx, g.ly / g.ny, g.lz / g.nz};
     for (int ax = 0; ax < 3; ax++)
         for (int m = 0; m < 3; m++) a.c1[ax][m] = (T)(W1[m] / h[ax]);
     for (int i = 0; i < 3; i++) a.bext[i] = (T)ctx->bext[i];
-    for (int q = 0; q < AC_NFIELDS; q++) a.in[q] = (const T*)ctx->field_ptr(ctx->cur, q);
+    for (int q = 0; q < AC_NFIELDS; q++) a.in[q] = ctx->field_ptr(ctx->cur, q);
     a.partial = (ac::RedVals*)(ctx->ws + ctx->cv.partial_off);
     ac::RedVals* result = (ac::RedVals*)(ctx->ws + ctx->cv.result_off);
     const long rows = (long)L.ny * L.nz;
     const int blocks = (int)std::min<long>(rows, RED_BLOCKS);
-    ac::reduce_stage1_kernel<T><<<blocks, 256, 0, ctx->stream>>>(a);
+    if (ctx->packed)
+        ac::reduce_stage1_kernel<T, 2><<<blocks, 256, 0, ctx->stream>>>(a);
+    else
+        ac::reduce_stage1_kernel<T, 1><<<blocks, 256, 0, ctx->stream>>>(a);
     ac::reduce_stage2_kernel<<<1, 256, 0, ctx->stream>>>(a.partial, blocks, result);
     ctx->launches += 2;
     AC_CUDA(cudaGetLastError());
     AC_CUDA(cudaMemcpyAsync(ctx->host_result, result, sizeof(ac::RedVals), cudaMemcpyDeviceToHost, ctx->stream));
     AC_CUDA(cudaStreamSynchronize(ctx->stream));
     const ac::RedVals& r = *ctx->host_result;
-    const double ncell = (double)L.nx * L.ny * L.nz;
+    const double ncell = (double)g.nx * g.ny * g.nz;
     out->urms = std::sqrt(r.su / ncell);
     out->umax = std::sqrt(r.mu);
     out->brms = std::sqrt(r.sb / ncell);
@@ -329,9 +427,70 @@ extern "C" {
 
 size_t ac_workspace_bytes(const ac_grid* grid, ac_dtype dtype) {
     if (!grid_ok(grid) || (dtype != AC_F32 && dtype != AC_F64)) return 0;
-    ac::Layout L = ac::make_layout(grid->nx, grid->ny, grid->nz, elem_size(dtype));
-    return carve(L, dtype).total;
+    // large enough for either device layout of this dtype (a context may switch variants)
+    size_t total = carve(layout_for(grid, dtype, false), store_elem_size(dtype, false), elem_size(dtype), grid->nz).total;
+    if (dtype == AC_F32 && can_pack(grid))
+        total = std::max(total, carve(layout_for(grid, dtype, true), 8, 4, grid->nz).total);
+    return total;
 }
+
+}  // extern "C"
+
+namespace {
+
+// choose the kernel and the device layout for the context's variant; builds the TMA maps
+int configure(ac_ctx* ctx) {
+    const ac_grid* g = &ctx->grid;
+    ctx->march = ctx->variant == 0 && (ctx->dtype == AC_F64 || can_pack(g));
+    ctx->packed = ctx->march && ctx->dtype == AC_F32;
+    ctx->L = layout_for(g, ctx->dtype, ctx->packed);
+    ctx->cv = carve(ctx->L, store_elem_size(ctx->dtype, ctx->packed), elem_size(ctx->dtype), g->nz);
+    ctx->loaded = false;
+    ctx->cur = 0;
+    if (!ctx->march) return AC_OK;
+    for (int b = 0; b < 2; b++) {
+        int rc = make_state_map(&ctx->map_in[b], ctx->field_ptr(b, 0), ctx->L, ac::M_WX, ac::M_WY);
+        if (rc == AC_OK) rc = make_state_map(&ctx->map_prev[b], ctx->field_ptr(b, 0), ctx->L, ac::M_TX, ac::M_TY);
+        if (rc != AC_OK) return rc;
+    }
+    cudaError_t ea = ctx->dtype == AC_F64
+                         ? cudaFuncSetAttribute(ac::substep_march_kernel<double>,
+                                                cudaFuncAttributeMaxDynamicSharedMemorySize, ac::M_SMEM_BYTES)
+                         : cudaFuncSetAttribute(ac::substep_march_kernel<float>,
+                                                cudaFuncAttributeMaxDynamicSharedMemorySize, ac::M_SMEM_BYTES);
+    if (ea != cudaSuccess) return cuda_fail(ea, "cudaFuncSetAttribute(march kernel smem)");
+    // z chunks: every chunk re-reads 6 planes, every wave of CTAs costs (planes + 6) iterations;
+    // pick the chunk count that minimises waves x (planes per chunk + 6)
+    const int nzp = ctx->L.nz;
+    const long tiles = (long)((ctx->L.nx + ac::M_TX - 1) / ac::M_TX) * ((ctx->L.ny + ac::M_TY - 1) / ac::M_TY);
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
+    long best_cost = -1;
+    int best_n = 1;
+    for (int n = 1; n <= 64; n++) {
+        const int cz = (nzp + n - 1) / n;
+        if (cz > ac::M_CZMAX) continue;
+        if (cz < 4 && n > 1) break;
+        const int nn = (nzp + cz - 1) / cz;
+        const long waves = (tiles * nn + sms - 1) / sms;
+        const long cost = waves * (cz + 6);
+        if (best_cost < 0 || cost < best_cost) {
+            best_cost = cost;
+            best_n = nn;
+            ctx->cz = cz;
+        }
+    }
+    ctx->nchunks = best_n;
+    if (const char* e = getenv("AC_MARCH_CZ")) {
+        ctx->cz = std::min(ac::M_CZMAX, std::max(1, atoi(e)));
+        ctx->nchunks = (nzp + ctx->cz - 1) / ctx->cz;
+    }
+    return AC_OK;
+}
+
+}  // namespace
+
+extern "C" {
 
 int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double eta, double cs, double k_f,
             double helicity, void* workspace_dev, void* cuda_stream) {
@@ -348,8 +507,8 @@ int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double
     cudaDeviceProp prop;
     AC_CUDA(cudaGetDeviceProperties(&prop, dev));
     if (prop.major != 10) {
-        snprintf(g_cuda_err, sizeof(g_cuda_err), "device %s is sm_%d%d; this library is built for sm_100a only", prop.name,
-                 prop.major, prop.minor);
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "device %.160s is sm_%d%d; this library is built for sm_100a only",
+                 prop.name, prop.major, prop.minor);
         return AC_ECUDA;
     }
 
@@ -366,57 +525,34 @@ int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double
     ctx->c_u = 0.4;
     ctx->c_nu = 0.25;
     ctx->variant = 0;
-    ctx->L = ac::make_layout(grid->nx, grid->ny, grid->nz, elem_size(dtype));
-    ctx->cv = carve(ctx->L, dtype);
     ctx->stream = (cudaStream_t)cuda_stream;
-    ctx->cur = 0;
-    ctx->loaded = false;
     ctx->launches = 0;
     ctx->host_result = nullptr;
-    ctx->shell = nullptr;
+    ctx->cz = 0;
+    ctx->nchunks = 1;
     if (workspace_dev) {
         ctx->ws = (char*)workspace_dev;
         ctx->owns_ws = false;
     } else {
         void* p = nullptr;
-        cudaError_t e = cudaMalloc(&p, ctx->cv.total);
+        cudaError_t e = cudaMalloc(&p, ac_workspace_bytes(grid, dtype));
         if (e != cudaSuccess) {
             cudaGetLastError();
-            delete ctx->shell;
             delete ctx;
             return e == cudaErrorMemoryAllocation ? AC_ENOMEM : cuda_fail(e, "cudaMalloc(workspace)");
         }
         ctx->ws = (char*)p;
         ctx->owns_ws = true;
     }
-    {
-        int rc;
-        const size_t es = elem_size(dtype);
-        const int wx = dtype == AC_F64 ? RingF64::WX : RingF32::WX, wy = dtype == AC_F64 ? RingF64::WY : RingF32::WY;
-        rc = make_state_map(&ctx->map[0], ctx->field_ptr(0, 0), ctx->L, es, wx, wy);
-        if (rc == AC_OK) rc = make_state_map(&ctx->map[1], ctx->field_ptr(1, 0), ctx->L, es, wx, wy);
-        cudaError_t ea = dtype == AC_F64
-                             ? cudaFuncSetAttribute(ac::substep_ring_kernel<double, RingF64>,
-                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, RingF64::SMEM_BYTES)
-                             : cudaFuncSetAttribute(ac::substep_ring_kernel<float, RingF32>,
-                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, RingF32::SMEM_BYTES);
-        if (rc == AC_OK && ea != cudaSuccess) rc = cuda_fail(ea, "cudaFuncSetAttribute(ring kernel smem)");
-        if (rc != AC_OK) {
-            if (ctx->owns_ws) cudaFree(ctx->ws);
-            delete ctx->shell;
-            delete ctx;
-            return rc;
-        }
-        // z chunk: long enough to amortise the 6 halo planes, short enough for >= ~8 waves of CTAs
-        ctx->cz = 64;
-        if (const char* e = getenv("AC_RING_CZ")) ctx->cz = std::max(1, atoi(e));
+    int rc = configure(ctx);
+    if (rc == AC_OK) {
+        cudaError_t e = cudaMallocHost((void**)&ctx->host_result, sizeof(ac::RedVals));
+        if (e != cudaSuccess) rc = cuda_fail(e, "cudaMallocHost");
     }
-    cudaError_t e = cudaMallocHost((void**)&ctx->host_result, sizeof(ac::RedVals));
-    if (e != cudaSuccess) {
+    if (rc != AC_OK) {
         if (ctx->owns_ws) cudaFree(ctx->ws);
-        delete ctx->shell;
         delete ctx;
-        return cuda_fail(e, "cudaMallocHost");
+        return rc;
     }
     *out = ctx;
     return AC_OK;
@@ -545,8 +681,11 @@ int ac_set_cfl(ac_ctx* ctx, double c_u, double c_nu) {
 int ac_set_variant(ac_ctx* ctx, int variant) {
     if (!ctx) return AC_EINVAL;
     if (variant != 0 && variant != 1) return AC_EINVAL;
+    if (variant == ctx->variant) return AC_OK;
+    // the variants use different device layouts in fp32: a loaded state would have to be re-packed
+    cudaStreamSynchronize(ctx->stream);
     ctx->variant = variant;
-    return AC_OK;
+    return configure(ctx);
 }
 
 long long ac_launch_count(const ac_ctx* ctx) { return ctx ? ctx->launches : 0; }
@@ -556,7 +695,6 @@ void ac_free(ac_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     if (ctx->owns_ws) cudaFree(ctx->ws);
     if (ctx->host_result) cudaFreeHost(ctx->host_result);
-    delete ctx->shell;
     delete ctx;
 }
 

@@ -35,6 +35,35 @@ __global__ void unpack_kernel(const T* __restrict__ padded, T* __restrict__ dens
     dense[(size_t)x + (size_t)L.nx * ((size_t)y + (size_t)L.ny * (size_t)z)] = padded[L.idx(x, y, z)];
 }
 
+// packed fp32 pairs (vec2.cuh): element (x, y, zp) = (cell z = zp, cell z = zp + nz/2); L is the layout in
+// 8-byte elements with L.nz = nz/2 planes.  Ghost planes come out lane-swapped by construction.
+__global__ void pack_pairs_kernel(const float* __restrict__ dense, float2* __restrict__ padded, Layout L, int nz_full) {
+    const int px = blockIdx.x * blockDim.x + threadIdx.x - R;
+    const int py = blockIdx.y * blockDim.y + threadIdx.y - R;
+    const int pz = blockIdx.z - R;
+    if (px >= L.nx + R || py >= L.ny + R) return;
+    int sx = px < 0 ? px + L.nx : (px >= L.nx ? px - L.nx : px);
+    int sy = py < 0 ? py + L.ny : (py >= L.ny ? py - L.ny : py);
+    int z0 = pz, z1 = pz + L.nz;
+    z0 = z0 < 0 ? z0 + nz_full : (z0 >= nz_full ? z0 - nz_full : z0);
+    z1 = z1 < 0 ? z1 + nz_full : (z1 >= nz_full ? z1 - nz_full : z1);
+    const size_t row = (size_t)sx + (size_t)L.nx * (size_t)sy;
+    const size_t plane = (size_t)L.nx * L.ny;
+    padded[L.idx(px, py, pz)] = make_float2(dense[row + plane * z0], dense[row + plane * z1]);
+}
+
+__global__ void unpack_pairs_kernel(const float2* __restrict__ padded, float* __restrict__ dense, Layout L) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= L.nx || y >= L.ny) return;
+    const float2 v = padded[L.idx(x, y, z)];
+    const size_t row = (size_t)x + (size_t)L.nx * (size_t)y;
+    const size_t plane = (size_t)L.nx * L.ny;
+    dense[row + plane * z] = v.x;
+    dense[row + plane * (z + L.nz)] = v.y;
+}
+
 // ------------------------------------------------------------------------------------------------
 // forcing tables (S7): cos/sin of k_a x_a per axis, phase folded into the z table.
 // layout: [cx(nx) sx(nx) cy(ny) sy(ny) cz(nz) sz(nz)]
@@ -196,15 +225,26 @@ __device__ __forceinline__ RedVals block_reduce(RedVals v) {
 
 template <typename T>
 struct ReduceArgs {
-    const T* in[NFIELDS];
-    Layout L;
+    const void* in[NFIELDS];   // T elements, or float2 pairs when LANES == 2
+    Layout L;                  // layout in storage elements
     T c1[3][3];
     T bext[3];
     RedVals* partial;
 };
 
-// stage 1: each block owns a fixed set of (y, z) rows; one partial per block
-template <typename T>
+template <typename T, int LANES>
+__device__ __forceinline__ void red_load(const void* base, size_t i, T (&v)[LANES]) {
+    if (LANES == 1) {
+        v[0] = ((const T*)base)[i];
+    } else {
+        const float2 t = ((const float2*)base)[i];
+        v[0] = (T)t.x;
+        v[LANES - 1] = (T)t.y;
+    }
+}
+
+// stage 1: each block owns a fixed set of (y, z) rows; one partial per block.  LANES = 2: packed fp32 pairs.
+template <typename T, int LANES>
 __global__ void __launch_bounds__(256) reduce_stage1_kernel(const __grid_constant__ ReduceArgs<T> a) {
     const Layout& L = a.L;
     RedVals acc = red_identity();
@@ -214,29 +254,54 @@ __global__ void __launch_bounds__(256) reduce_stage1_kernel(const __grid_constan
         const int y = (int)(row % L.ny), z = (int)(row / L.ny);
         for (int x = threadIdx.x; x < L.nx; x += blockDim.x) {
             const size_t c0 = L.idx(x, y, z);
-            const T ux = a.in[UX][c0], uy = a.in[UY][c0], uz = a.in[UZ][c0];
-            const T l = a.in[LNRHO][c0];
-            auto d = [&](int q, long stride, int axis) -> T {
-                const T* p = a.in[q] + c0;
-                T r = a.c1[axis][0] * (p[stride] - p[-stride]);
-                r = fma_<T>(a.c1[axis][1], p[2 * stride] - p[-2 * stride], r);
-                r = fma_<T>(a.c1[axis][2], p[3 * stride] - p[-3 * stride], r);
-                return r;
+            T ux[LANES], uy[LANES], uz[LANES], l[LANES], ax[LANES], ay[LANES], az[LANES];
+            red_load<T, LANES>(a.in[UX], c0, ux);
+            red_load<T, LANES>(a.in[UY], c0, uy);
+            red_load<T, LANES>(a.in[UZ], c0, uz);
+            red_load<T, LANES>(a.in[LNRHO], c0, l);
+            red_load<T, LANES>(a.in[AX], c0, ax);
+            red_load<T, LANES>(a.in[AY], c0, ay);
+            red_load<T, LANES>(a.in[AZ], c0, az);
+            // first derivative of field q along an axis with element stride `stride`
+            auto d = [&](int q, long stride, int axis, T (&r)[LANES]) {
+                T p1[LANES], m1[LANES], p2[LANES], m2[LANES], p3[LANES], m3[LANES];
+                red_load<T, LANES>(a.in[q], c0 + stride, p1);
+                red_load<T, LANES>(a.in[q], c0 - stride, m1);
+                red_load<T, LANES>(a.in[q], c0 + 2 * stride, p2);
+                red_load<T, LANES>(a.in[q], c0 - 2 * stride, m2);
+                red_load<T, LANES>(a.in[q], c0 + 3 * stride, p3);
+                red_load<T, LANES>(a.in[q], c0 - 3 * stride, m3);
+#pragma unroll
+                for (int i = 0; i < LANES; i++) {
+                    T v = a.c1[axis][0] * (p1[i] - m1[i]);
+                    v = fma_<T>(a.c1[axis][1], p2[i] - m2[i], v);
+                    r[i] = fma_<T>(a.c1[axis][2], p3[i] - m3[i], v);
+                }
             };
-            const T bx = d(AZ, pitch, 1) - d(AY, plane, 2) + a.bext[0];
-            const T by = d(AX, plane, 2) - d(AZ, 1, 0) + a.bext[1];
-            const T bz = d(AY, 1, 0) - d(AX, pitch, 1) + a.bext[2];
-            const double u2 = (double)ux * ux + (double)uy * uy + (double)uz * uz;
-            const double b2 = (double)bx * bx + (double)by * by + (double)bz * bz;
-            acc.su += u2;
-            acc.sb += b2;
-            acc.mu = fmax(acc.mu, u2);
-            acc.mb = fmax(acc.mb, b2);
-            acc.lmin = fmin(acc.lmin, (double)l);
-            acc.lmax = fmax(acc.lmax, (double)l);
-            // a non-finite ln rho or A would hide in fmin/fmax: fold it into the sums
-            const double chk = (double)l + (double)a.in[AX][c0] + (double)a.in[AY][c0] + (double)a.in[AZ][c0];
-            if (!isfinite(chk)) acc.su += chk;
+            T azy[LANES], ayz[LANES], axz[LANES], azx[LANES], ayx[LANES], axy[LANES];
+            d(AZ, pitch, 1, azy);
+            d(AY, plane, 2, ayz);
+            d(AX, plane, 2, axz);
+            d(AZ, 1, 0, azx);
+            d(AY, 1, 0, ayx);
+            d(AX, pitch, 1, axy);
+#pragma unroll
+            for (int i = 0; i < LANES; i++) {
+                const T bx = azy[i] - ayz[i] + a.bext[0];
+                const T by = axz[i] - azx[i] + a.bext[1];
+                const T bz = ayx[i] - axy[i] + a.bext[2];
+                const double u2 = (double)ux[i] * ux[i] + (double)uy[i] * uy[i] + (double)uz[i] * uz[i];
+                const double b2 = (double)bx * bx + (double)by * by + (double)bz * bz;
+                acc.su += u2;
+                acc.sb += b2;
+                acc.mu = fmax(acc.mu, u2);
+                acc.mb = fmax(acc.mb, b2);
+                acc.lmin = fmin(acc.lmin, (double)l[i]);
+                acc.lmax = fmax(acc.lmax, (double)l[i]);
+                // a non-finite ln rho or A would hide in fmin/fmax: fold it into the sums
+                const double chk = (double)l[i] + (double)ax[i] + (double)ay[i] + (double)az[i];
+                if (!isfinite(chk)) acc.su += chk;
+            }
         }
     }
     acc = block_reduce(acc);

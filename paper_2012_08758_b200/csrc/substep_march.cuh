@@ -1,0 +1,573 @@
+// Fused RK substep, variant "scatter-march" (the default).
+//
+// What it computes: exactly the substep of mhd_cell.cuh / the oracle - Eq. 1-3 right-hand sides
+// (PAPER.md:166-170), forcing Eq. 4, 6th-order radius-3 central differences
+// (readings G1-G3), j = grad div A - lap A (G4), the 2N-RK3 update in difference
+// form (G7) - with the sums re-associated as follows.
+//
+// A CTA owns a 16 x 8 tile of (x, y) columns and marches along z.  Plane p (all 7 fields, tile +
+// halo) is brought into a shared-memory ring by ONE 4-D TMA box load; a second box brings the
+// previous-state values (2N register) of the plane that is finalised in the same iteration.
+// Each column is served by two threads ("roles"): U carries ln rho and u, A carries A.
+//
+// When plane p arrives a thread loads only the IN-PLANE neighbourhood of its cell (centre, x row,
+// y column, xy diagonals) and forms  dx_m = f(x+m) - f(x-m), dy_m, sx_m = f(x+m) + f(x-m), sy_m.
+// These give d_x, d_y, d_xx, d_yy, d_xy of cell p directly.  Everything that couples planes is
+// SCATTERED into register accumulators of the pending cells p-3 .. p+3 ("levels" r = 0 .. 6,
+// r = 3 being plane p itself):
+//     d_z f (z)  = sum_m c1z_m [f(z+m) - f(z-m)]            <- centre value of plane p, weight -/+ c1z_m
+//     d_zz f (z) = c20z f(z) + sum_m c2z_m [f(z+m) + f(z-m)]
+//     d_xz f (z) = sum_m cm_m [dx_m(z+m) - dx_m(z-m)]       (G2's 12 points, re-associated)
+//     d_yz f (z) = sum_m cm_m [dy_m(z+m) - dy_m(z-m)]
+// so a cell needs 139 shared-memory loads instead of 277 and a mixed z derivative costs 6 FMAs on
+// differences the first derivatives need anyway.  Quantities that enter the equations linearly
+// are accumulated already combined: L_i = lap u_i + 1/3 (grad div u)_i, lap A_i,
+// J_i = (grad div A - lap A)_i, B_i.  The cell at level 0 (plane p-3) is complete after plane p
+// has been scattered; it is then finalised: non-linear terms, forcing, 2N update, store (with the
+// periodic ghost images of boundary cells).
+//
+// Synchronisation: no block-wide barrier in the loop.  full[slot] (TMA transaction bytes) and
+// done[iteration] (one arrival per warp) mbarriers; lane 0 of warp 0 refills ring slots 3 planes
+// ahead once every warp has finished the iteration that last read them.  The A role hands
+// (j x B) to the U role of the same columns through a mailbox with one mbarrier per warp pair.
+//
+// Element type E (vec2.cuh): double, or f2 = two fp32 cells (z, z + nz/2) per element.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "layout.cuh"
+#include "vec2.cuh"
+
+namespace ac {
+
+constexpr int M_TX = 16, M_TY = 8, M_COLS = M_TX * M_TY, M_THREADS = 2 * M_COLS;
+constexpr int M_HX = 4;                  // x halo of the tile in shared memory (>= R; 32 bytes keeps TMA boxes aligned)
+constexpr int M_WX = M_TX + 2 * M_HX;    // 24
+constexpr int M_WY = M_TY + 2 * R;       // 14
+constexpr int M_PLANE = M_WX * M_WY;     // elements per field per plane slot
+constexpr int M_NP = 8;                  // ring slots: planes p-3 .. p resident, p+1 .. p+3 in flight
+constexpr int M_NPP = 5;                 // previous-state ring slots
+constexpr int M_ND = 5;                  // mailbox depth
+constexpr int M_LEAD = 3;                // planes issued ahead of the one being processed
+constexpr int M_CZMAX = 512;             // longest z chunk (bounds the z phase table in shared memory)
+constexpr int M_NF = 7;
+
+constexpr int M_SLOT_BYTES = M_NF * M_PLANE * 8;        // 18816 (multiple of 128)
+constexpr int M_PSLOT_BYTES = M_NF * M_COLS * 8;        // 7168
+constexpr int M_MBOX_BYTES = 3 * M_COLS * 8;            // 3072 per depth
+constexpr int M_OFF_PREV = M_NP * M_SLOT_BYTES;
+constexpr int M_OFF_MBOX = M_OFF_PREV + M_NPP * M_PSLOT_BYTES;
+constexpr int M_OFF_ZTAB = M_OFF_MBOX + M_ND * M_MBOX_BYTES;
+constexpr int M_OFF_BARS = M_OFF_ZTAB + M_CZMAX * 2 * 8;
+constexpr int M_NBARS = 2 * M_NP + 4 * M_ND;
+constexpr int M_SMEM_BYTES = M_OFF_BARS + M_NBARS * 8 + 128;   // + slack for the 128-byte alignment of the base
+static_assert(M_SLOT_BYTES % 128 == 0 && M_PSLOT_BYTES % 128 == 0, "TMA destinations must stay 128-byte aligned");
+static_assert(M_SMEM_BYTES <= 232448, "exceeds the 227 KB of shared memory a CTA may use");
+
+// Weights with the grid spacing (and, for the U role, the 1/3 of grad div and the 4/3 of the
+// diagonal second derivative) folded in; n* = negated copies (packed fp32 has no negate modifier in PTX).
+template <typename E>
+struct MarchCoef {
+    E c1x[3], c1y[3], c1z[3], nc1z[3];
+    // U role: L_i = lap u_i + 1/3 (grad div u)_i
+    E w2x[3][3], w2y[3][3], w2z[3][3], w20[3];      // [component][m-1]; w20 = centre weight summed over the axes
+    E cm3xy[3], cm3xz[3], ncm3xz[3], cm3yz[3], ncm3yz[3];
+    // A role
+    E c2x[3], c2y[3], c2z[3], nc2x[3], nc2y[3], nc2z[3];
+    E c20all, nc20yz, nc20xz, nc20xy;
+    E cmxy[3], cmxz[3], ncmxz[3], cmyz[3], ncmyz[3];
+    // physics and time stepping
+    E nu, eta, ncs2, bext[3], rk_a, rk_b, fre[3], nfim[3], n23;
+};
+
+template <typename T>
+struct MarchArgs {
+    using E = typename ElemOf<T>::E;
+    E* out[M_NF];        // buffer 1-cur: previous state on entry (read through map_prev), new state on exit
+    const T* ftab;       // forcing tables [cx(nx) sx(nx) cy(ny) sy(ny) cz(nzfull) sz(nzfull)]
+    Layout L;            // layout in 8-byte elements; L.nz = number of (packed) planes
+    int nz_full;         // planes of the caller's grid (= L.nz, or 2 L.nz for packed fp32)
+    int cz;              // planes per z chunk (<= M_CZMAX)
+    int substep;
+    int has_forcing;
+    MarchCoef<E> c;
+};
+
+// ---- mbarrier / TMA primitives -------------------------------------------------------------------
+__device__ __forceinline__ uint32_t m_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void m_bar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(m_smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void m_bar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(m_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void m_bar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(m_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void m_bar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "MWAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra MDONE_%=;\n"
+        "bra MWAIT_%=;\n"
+        "MDONE_%=:\n"
+        "}\n" ::"r"(m_smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void m_tma_load_4d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2,
+                                              int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];" ::
+            "r"(m_smem_u32(dst)),
+        "l"(map), "r"(m_smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
+
+// ---- small stencil helpers -----------------------------------------------------------------------
+template <typename E>
+__device__ __forceinline__ E m_dot3(const E (&c)[3], const E (&d)[3]) {
+    E r = vmul(c[0], d[0]);
+    r = vfma(c[1], d[1], r);
+    r = vfma(c[2], d[2], r);
+    return r;
+}
+template <typename E>
+__device__ __forceinline__ E m_dot3(const E (&c)[3], const E (&d)[3], E r) {
+    r = vfma(c[0], d[0], r);
+    r = vfma(c[1], d[1], r);
+    r = vfma(c[2], d[2], r);
+    return r;
+}
+// differences and sums along x (stride 1) or y (stride M_WX) around p
+template <typename E, int STRIDE>
+__device__ __forceinline__ void m_diff_sum(const E* p, E (&d)[3], E (&s)[3]) {
+#pragma unroll
+    for (int m = 1; m <= 3; m++) {
+        const E a = p[m * STRIDE], b = p[-m * STRIDE];
+        d[m - 1] = vsub(a, b);
+        s[m - 1] = vadd(a, b);
+    }
+}
+template <typename E, int STRIDE>
+__device__ __forceinline__ void m_diff(const E* p, E (&d)[3]) {
+#pragma unroll
+    for (int m = 1; m <= 3; m++) d[m - 1] = vsub(p[m * STRIDE], p[-m * STRIDE]);
+}
+// in-plane bidiagonal mixed derivative (G2) with weights cm
+template <typename E>
+__device__ __forceinline__ E m_mixxy(const E* p, const E (&cm)[3]) {
+    E r;
+#pragma unroll
+    for (int m = 1; m <= 3; m++) {
+        const E s = vsub(vadd(p[m * M_WX + m], p[-m * M_WX - m]), vadd(p[-m * M_WX + m], p[m * M_WX - m]));
+        r = (m == 1) ? vmul(cm[0], s) : vfma(cm[m - 1], s, r);
+    }
+    return r;
+}
+// scatter v into the levels m below (r = 3 - m, weight cdn) and m above (r = 3 + m, weight cup) plane p
+#define M_SCAT(acc, m, cdn, cup, v)                           \
+    do {                                                      \
+        acc[3 - (m)] = vfma((cdn), (v), acc[3 - (m)]);        \
+        acc[3 + (m)] = vfma((cup), (v), acc[3 + (m)]);        \
+    } while (0)
+
+// new value of a cell and its periodic ghost images; z images of packed pairs swap lanes
+template <typename E>
+__device__ __forceinline__ void m_store(E* __restrict__ o, const Layout& L, int x, int y, int z, E v, bool edge) {
+    o[L.idx(x, y, z)] = v;
+    if (!edge) return;
+    int xs[2] = {x, x}, ys[2] = {y, y}, zs[3] = {z, z, z};
+    int cx = 1, cy = 1, cz = 1;
+    if (x < R) xs[cx++] = x + L.nx; else if (x >= L.nx - R) xs[cx++] = x - L.nx;
+    if (y < R) ys[cy++] = y + L.ny; else if (y >= L.ny - R) ys[cy++] = y - L.ny;
+    if (z < R) zs[cz++] = z + L.nz;
+    if (z >= L.nz - R) zs[cz++] = z - L.nz;      // both can hold when a packed grid has fewer than 6 planes
+    const E vs = vswap(v);
+    for (int k = 0; k < cz; k++)
+        for (int j = 0; j < cy; j++)
+            for (int i = 0; i < cx; i++)
+                if (i + j + k) o[L.idx(xs[i], ys[j], zs[k])] = k ? vs : v;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(M_THREADS, 1)
+    substep_march_kernel(const __grid_constant__ MarchArgs<T> a, const __grid_constant__ CUtensorMap map_in,
+                         const __grid_constant__ CUtensorMap map_prev) {
+    using E = typename ElemOf<T>::E;
+    extern __shared__ unsigned char m_smem_raw[];
+    unsigned char* smem = (unsigned char*)(((uintptr_t)m_smem_raw + 127) & ~(uintptr_t)127);
+    E* ztab = (E*)(smem + M_OFF_ZTAB);
+    uint64_t* full = (uint64_t*)(smem + M_OFF_BARS);
+    uint64_t* done = full + M_NP;
+    uint64_t* mfull = done + M_NP;     // [pair][depth]
+
+    const Layout& L = a.L;
+    const MarchCoef<E>& c = a.c;
+    const int tid = threadIdx.x;
+    const int role = tid >> 7;              // 0 = U (ln rho, u), 1 = A
+    const int col = tid & (M_COLS - 1);
+    const int tx = col & (M_TX - 1), ty = col >> 4;
+    const int lane = tid & 31;
+    const int pair = (tid >> 5) & 3;        // U warp w and A warp w + 4 serve the same 32 columns
+    const int x0 = blockIdx.x * M_TX, y0 = blockIdx.y * M_TY;
+    const int zs = blockIdx.z * a.cz;
+    const int ze = min(zs + a.cz, L.nz);
+    const int niter = ze - zs + 2 * R;      // planes zs-3 .. ze+2
+    const int x = x0 + tx, y = y0 + ty;
+    const bool valid = (x < L.nx) && (y < L.ny);
+    const bool edge_xy = (x < R) | (x >= L.nx - R) | (y < R) | (y >= L.ny - R);
+    const bool with_prev = a.substep != 0;
+
+    if (tid == 0) {
+        for (int s = 0; s < M_NP; s++) {
+            m_bar_init(&full[s], 1);
+            m_bar_init(&done[s], M_THREADS / 32);
+        }
+        for (int s = 0; s < 4 * M_ND; s++) m_bar_init(&mfull[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    // z phase table of this chunk: (cos, sin)(k_z z + phase) per level, lanes = (z, z + nz/2) for packed pairs
+    if (a.has_forcing) {
+        const T* tz = a.ftab + 2 * L.nx + 2 * L.ny;
+        for (int i = tid; i < ze - zs; i += M_THREADS) {
+            const int z = zs + i;
+            const int z2 = (ElemOf<T>::LANES == 2) ? z + L.nz : z;
+            ztab[2 * i] = vmake(tz[z], tz[z2]);
+            ztab[2 * i + 1] = vmake(tz[a.nz_full + z], tz[a.nz_full + z2]);
+        }
+    }
+    __syncthreads();
+
+    // iteration k processes plane zs - 3 + k and finalises level zs - 6 + k
+    auto issue = [&](int k) {
+        const int slot = k % M_NP;
+        const bool fin = with_prev && k >= 2 * R;
+        m_bar_expect_tx(&full[slot], (uint32_t)(M_SLOT_BYTES + (fin ? M_PSLOT_BYTES : 0)));
+        m_tma_load_4d(smem + slot * M_SLOT_BYTES, &map_in, &full[slot], x0 - M_HX + L.gx, y0, zs + k, 0);
+        if (fin)
+            m_tma_load_4d(smem + M_OFF_PREV + (k % M_NPP) * M_PSLOT_BYTES, &map_prev, &full[slot], x0 + L.gx, y0 + R,
+                          zs + k - R, 0);
+    };
+    if (tid == 0)
+        for (int k = 0; k < M_LEAD && k < niter; k++) issue(k);
+
+    const int cell_off = (ty + R) * M_WX + tx + M_HX;
+
+    // forcing: cos/sin of k_x x + k_y y, constant along the march
+    E cxy = vzero<E>(), sxy = vzero<E>();
+    if (role == 0 && a.has_forcing && valid) {
+        const T cx_ = a.ftab[x], sx_ = a.ftab[L.nx + x];
+        const T cy_ = a.ftab[2 * L.nx + y], sy_ = a.ftab[2 * L.nx + L.ny + y];
+        cxy = Splat<E>::of((double)(cx_ * cy_ - sx_ * sy_));
+        sxy = Splat<E>::of((double)(sx_ * cy_ + cx_ * sy_));
+    }
+
+    if (role == 0) {
+        // ======================================= U role ========================================
+        E gz[7], Gxz[7], Gyz[7], Gzz[7], Lx[7], Ly[7], Lz[7];     // z-coupled accumulators, levels 0..6
+        E gx[4], gy[4], Gxx[4], Gxy[4], Gyx[4], Gyy[4], Gzx[4], Gzy[4];   // in-plane first derivatives, levels 0..3
+#pragma unroll
+        for (int r = 0; r < 7; r++) gz[r] = Gxz[r] = Gyz[r] = Gzz[r] = Lx[r] = Ly[r] = Lz[r] = vzero<E>();
+#pragma unroll
+        for (int r = 0; r < 4; r++) gx[r] = gy[r] = Gxx[r] = Gxy[r] = Gyx[r] = Gyy[r] = Gzx[r] = Gzy[r] = vzero<E>();
+
+        for (int k = 0; k < niter; k++) {
+            if (tid == 0 && k + M_LEAD < niter) {
+                if (k >= 2) m_bar_wait(&done[(k - 2) % M_NP], (uint32_t)(((k - 2) / M_NP) & 1));
+                issue(k + M_LEAD);
+            }
+            m_bar_wait(&full[k % M_NP], (uint32_t)((k / M_NP) & 1));
+            const E* pl = (const E*)(smem + (k % M_NP) * M_SLOT_BYTES) + cell_off;
+
+            gz[6] = Gxz[6] = Gyz[6] = Gzz[6] = Lx[6] = Ly[6] = Lz[6] = vzero<E>();
+            E d[3], s[3], e[3], t[3];
+            // ---- ln rho ----
+            {
+                const E* p = pl;
+                const E f0 = p[0];
+                m_diff<E, 1>(p, d);
+                m_diff<E, M_WX>(p, e);
+                gx[3] = m_dot3(c.c1x, d);
+                gy[3] = m_dot3(c.c1y, e);
+#pragma unroll
+                for (int m = 1; m <= 3; m++) M_SCAT(gz, m, c.c1z[m - 1], c.nc1z[m - 1], f0);
+            }
+            // ---- u_x: d_x, d_y; L_x in-plane; D_xy u_x -> L_y; D_xz u_x -> L_z ----
+            {
+                const E* p = pl + 1 * M_PLANE;
+                const E f0 = p[0];
+                m_diff_sum<E, 1>(p, d, s);
+                m_diff_sum<E, M_WX>(p, e, t);
+                Gxx[3] = m_dot3(c.c1x, d);
+                Gxy[3] = m_dot3(c.c1y, e);
+                E l = vfma(c.w20[0], f0, Lx[3]);
+                l = m_dot3(c.w2x[0], s, l);
+                Lx[3] = m_dot3(c.w2y[0], t, l);
+                Ly[3] = vadd(Ly[3], m_mixxy(p, c.cm3xy));
+#pragma unroll
+                for (int m = 1; m <= 3; m++) {
+                    M_SCAT(Gxz, m, c.c1z[m - 1], c.nc1z[m - 1], f0);
+                    M_SCAT(Lx, m, c.w2z[0][m - 1], c.w2z[0][m - 1], f0);
+                    M_SCAT(Lz, m, c.cm3xz[m - 1], c.ncm3xz[m - 1], d[m - 1]);
+                }
+            }
+            // ---- u_y: D_xy u_y -> L_x; D_yz u_y -> L_z ----
+            {
+                const E* p = pl + 2 * M_PLANE;
+                const E f0 = p[0];
+                m_diff_sum<E, 1>(p, d, s);
+                m_diff_sum<E, M_WX>(p, e, t);
+                Gyx[3] = m_dot3(c.c1x, d);
+                Gyy[3] = m_dot3(c.c1y, e);
+                E l = vfma(c.w20[1], f0, Ly[3]);
+                l = m_dot3(c.w2x[1], s, l);
+                Ly[3] = m_dot3(c.w2y[1], t, l);
+                Lx[3] = vadd(Lx[3], m_mixxy(p, c.cm3xy));
+#pragma unroll
+                for (int m = 1; m <= 3; m++) {
+                    M_SCAT(Gyz, m, c.c1z[m - 1], c.nc1z[m - 1], f0);
+                    M_SCAT(Ly, m, c.w2z[1][m - 1], c.w2z[1][m - 1], f0);
+                    M_SCAT(Lz, m, c.cm3yz[m - 1], c.ncm3yz[m - 1], e[m - 1]);
+                }
+            }
+            // ---- u_z: D_xz u_z -> L_x; D_yz u_z -> L_y ----
+            {
+                const E* p = pl + 3 * M_PLANE;
+                const E f0 = p[0];
+                m_diff_sum<E, 1>(p, d, s);
+                m_diff_sum<E, M_WX>(p, e, t);
+                Gzx[3] = m_dot3(c.c1x, d);
+                Gzy[3] = m_dot3(c.c1y, e);
+                E l = vfma(c.w20[2], f0, Lz[3]);
+                l = m_dot3(c.w2x[2], s, l);
+                Lz[3] = m_dot3(c.w2y[2], t, l);
+#pragma unroll
+                for (int m = 1; m <= 3; m++) {
+                    M_SCAT(Gzz, m, c.c1z[m - 1], c.nc1z[m - 1], f0);
+                    M_SCAT(Lz, m, c.w2z[2][m - 1], c.w2z[2][m - 1], f0);
+                    M_SCAT(Lx, m, c.cm3xz[m - 1], c.ncm3xz[m - 1], d[m - 1]);
+                    M_SCAT(Ly, m, c.cm3yz[m - 1], c.ncm3yz[m - 1], e[m - 1]);
+                }
+            }
+
+            // ---- finalise level 0 = plane zs - 6 + k ----
+            if (k >= 2 * R) {
+                const int z = zs + k - 2 * R;
+                const E* pc = (const E*)(smem + ((k - R) % M_NP) * M_SLOT_BYTES) + cell_off;
+                const E lnrho = pc[0], ux = pc[M_PLANE], uy = pc[2 * M_PLANE], uz = pc[3 * M_PLANE];
+                const E g0 = gx[0], g1 = gy[0], g2 = gz[0];
+                const E divu = vadd(vadd(Gxx[0], Gyy[0]), Gzz[0]);
+                // Eq. 1
+                E rl = vmul(ux, g0);
+                rl = vfma(uy, g1, rl);
+                rl = vfma(uz, g2, rl);
+                rl = vneg(vadd(rl, divu));
+                const E rho_inv = vexpneg(lnrho);
+                // (j x B) from the A role of the same columns
+                const int u = k - 2 * R;
+                m_bar_wait(&mfull[pair * M_ND + u % M_ND], (uint32_t)((u / M_ND) & 1));
+                const E* mb = (const E*)(smem + M_OFF_MBOX + (u % M_ND) * M_MBOX_BYTES) + col;
+                const E jxb0 = mb[0], jxb1 = mb[M_COLS], jxb2 = mb[2 * M_COLS];
+                // forcing Eq. 4: f_i = re_i cos(theta) - im_i sin(theta)
+                E fc = vzero<E>(), fs = vzero<E>();
+                if (a.has_forcing) {
+                    const E cz_ = ztab[2 * (z - zs)], sz_ = ztab[2 * (z - zs) + 1];
+                    fc = vsub(vmul(cxy, cz_), vmul(sxy, sz_));
+                    fs = vfma(sxy, cz_, vmul(cxy, sz_));
+                }
+                // 2 S_ij g_j = (G_ij + G_ji) g_j - 2/3 div u g_i
+                const E sxy_ = vadd(Gxy[0], Gyx[0]), sxz_ = vadd(Gxz[0], Gzx[0]), syz_ = vadd(Gyz[0], Gzy[0]);
+                const E dd = vmul(c.n23, divu);
+                E sg0 = vmul(vadd(Gxx[0], Gxx[0]), g0);
+                sg0 = vfma(sxy_, g1, sg0);
+                sg0 = vfma(sxz_, g2, sg0);
+                sg0 = vfma(dd, g0, sg0);
+                E sg1 = vmul(sxy_, g0);
+                sg1 = vfma(vadd(Gyy[0], Gyy[0]), g1, sg1);
+                sg1 = vfma(syz_, g2, sg1);
+                sg1 = vfma(dd, g1, sg1);
+                E sg2 = vmul(sxz_, g0);
+                sg2 = vfma(syz_, g1, sg2);
+                sg2 = vfma(vadd(Gzz[0], Gzz[0]), g2, sg2);
+                sg2 = vfma(dd, g2, sg2);
+                // Eq. 2
+                E adv0 = vmul(ux, Gxx[0]);
+                adv0 = vfma(uy, Gxy[0], adv0);
+                adv0 = vfma(uz, Gxz[0], adv0);
+                E adv1 = vmul(ux, Gyx[0]);
+                adv1 = vfma(uy, Gyy[0], adv1);
+                adv1 = vfma(uz, Gyz[0], adv1);
+                E adv2 = vmul(ux, Gzx[0]);
+                adv2 = vfma(uy, Gzy[0], adv2);
+                adv2 = vfma(uz, Gzz[0], adv2);
+                E r0 = vfma(c.nu, vadd(Lx[0], sg0), vfma(jxb0, rho_inv, vsub(vmul(c.ncs2, g0), adv0)));
+                E r1 = vfma(c.nu, vadd(Ly[0], sg1), vfma(jxb1, rho_inv, vsub(vmul(c.ncs2, g1), adv1)));
+                E r2 = vfma(c.nu, vadd(Lz[0], sg2), vfma(jxb2, rho_inv, vsub(vmul(c.ncs2, g2), adv2)));
+                if (a.has_forcing) {
+                    r0 = vfma(c.fre[0], fc, vfma(c.nfim[0], fs, r0));
+                    r1 = vfma(c.fre[1], fc, vfma(c.nfim[1], fs, r1));
+                    r2 = vfma(c.fre[2], fc, vfma(c.nfim[2], fs, r2));
+                }
+                // 2N-RK3 update, difference form
+                E o0 = lnrho, o1 = ux, o2 = uy, o3 = uz;
+                if (with_prev) {
+                    const E* pp = (const E*)(smem + M_OFF_PREV + (k % M_NPP) * M_PSLOT_BYTES) + col;
+                    o0 = vfma(c.rk_a, vsub(lnrho, pp[0]), o0);
+                    o1 = vfma(c.rk_a, vsub(ux, pp[M_COLS]), o1);
+                    o2 = vfma(c.rk_a, vsub(uy, pp[2 * M_COLS]), o2);
+                    o3 = vfma(c.rk_a, vsub(uz, pp[3 * M_COLS]), o3);
+                }
+                o0 = vfma(c.rk_b, rl, o0);
+                o1 = vfma(c.rk_b, r0, o1);
+                o2 = vfma(c.rk_b, r1, o2);
+                o3 = vfma(c.rk_b, r2, o3);
+                if (valid) {
+                    const bool edge = edge_xy | (z < R) | (z >= L.nz - R);
+                    m_store<E>(a.out[0], L, x, y, z, o0, edge);
+                    m_store<E>(a.out[1], L, x, y, z, o1, edge);
+                    m_store<E>(a.out[2], L, x, y, z, o2, edge);
+                    m_store<E>(a.out[3], L, x, y, z, o3, edge);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) m_bar_arrive(&done[k % M_NP]);
+            // next plane: every pending level moves one step closer to completion
+#pragma unroll
+            for (int r = 0; r < 6; r++) {
+                gz[r] = gz[r + 1]; Gxz[r] = Gxz[r + 1]; Gyz[r] = Gyz[r + 1]; Gzz[r] = Gzz[r + 1];
+                Lx[r] = Lx[r + 1]; Ly[r] = Ly[r + 1]; Lz[r] = Lz[r + 1];
+            }
+#pragma unroll
+            for (int r = 0; r < 3; r++) {
+                gx[r] = gx[r + 1]; gy[r] = gy[r + 1]; Gxx[r] = Gxx[r + 1]; Gxy[r] = Gxy[r + 1];
+                Gyx[r] = Gyx[r + 1]; Gyy[r] = Gyy[r + 1]; Gzx[r] = Gzx[r + 1]; Gzy[r] = Gzy[r + 1];
+            }
+        }
+    } else {
+        // ======================================= A role ========================================
+        E Bx[7], By[7], Px[7], Py[7], Pz[7], Jx[7], Jy[7], Jz[7];   // P_i = lap A_i
+        E Bz[4];
+#pragma unroll
+        for (int r = 0; r < 7; r++) Bx[r] = By[r] = Px[r] = Py[r] = Pz[r] = Jx[r] = Jy[r] = Jz[r] = vzero<E>();
+#pragma unroll
+        for (int r = 0; r < 4; r++) Bz[r] = vzero<E>();
+
+        for (int k = 0; k < niter; k++) {
+            m_bar_wait(&full[k % M_NP], (uint32_t)((k / M_NP) & 1));
+            const E* pl = (const E*)(smem + (k % M_NP) * M_SLOT_BYTES) + cell_off;
+
+            Bx[6] = By[6] = Px[6] = Py[6] = Pz[6] = Jx[6] = Jy[6] = Jz[6] = vzero<E>();
+            E d[3], s[3], e[3], t[3];
+            // ---- A_x: B_z -= d_y A_x; lap; J_x -= (D_yy + D_zz) A_x; D_xy A_x -> J_y; D_xz A_x -> J_z; B_y += d_z A_x
+            {
+                const E* p = pl + 4 * M_PLANE;
+                const E f0 = p[0];
+                m_diff_sum<E, 1>(p, d, s);
+                m_diff_sum<E, M_WX>(p, e, t);
+                const E dyax = m_dot3(c.c1y, e);
+                const E px = m_dot3(c.c2x, s), py = m_dot3(c.c2y, t);
+                Px[3] = vadd(vfma(c.c20all, f0, Px[3]), vadd(px, py));
+                Jx[3] = vsub(vfma(c.nc20yz, f0, Jx[3]), py);
+                Jy[3] = vadd(Jy[3], m_mixxy(p, c.cmxy));
+                Bz[3] = vneg(dyax);
+#pragma unroll
+                for (int m = 1; m <= 3; m++) {
+                    M_SCAT(By, m, c.c1z[m - 1], c.nc1z[m - 1], f0);
+                    M_SCAT(Px, m, c.c2z[m - 1], c.c2z[m - 1], f0);
+                    M_SCAT(Jx, m, c.nc2z[m - 1], c.nc2z[m - 1], f0);
+                    M_SCAT(Jz, m, c.cmxz[m - 1], c.ncmxz[m - 1], d[m - 1]);
+                }
+            }
+            // ---- A_y: B_z += d_x A_y; lap; J_y -= (D_xx + D_zz) A_y; D_xy A_y -> J_x; D_yz A_y -> J_z; B_x -= d_z A_y
+            {
+                const E* p = pl + 5 * M_PLANE;
+                const E f0 = p[0];
+                m_diff_sum<E, 1>(p, d, s);
+                m_diff_sum<E, M_WX>(p, e, t);
+                Bz[3] = m_dot3(c.c1x, d, Bz[3]);
+                const E px = m_dot3(c.c2x, s), py = m_dot3(c.c2y, t);
+                Py[3] = vadd(vfma(c.c20all, f0, Py[3]), vadd(px, py));
+                Jy[3] = vsub(vfma(c.nc20xz, f0, Jy[3]), px);
+                Jx[3] = vadd(Jx[3], m_mixxy(p, c.cmxy));
+#pragma unroll
+                for (int m = 1; m <= 3; m++) {
+                    M_SCAT(Bx, m, c.nc1z[m - 1], c.c1z[m - 1], f0);
+                    M_SCAT(Py, m, c.c2z[m - 1], c.c2z[m - 1], f0);
+                    M_SCAT(Jy, m, c.nc2z[m - 1], c.nc2z[m - 1], f0);
+                    M_SCAT(Jz, m, c.cmyz[m - 1], c.ncmyz[m - 1], e[m - 1]);
+                }
+            }
+            // ---- A_z: B_x += d_y A_z; B_y -= d_x A_z; lap; J_z -= (D_xx + D_yy) A_z; D_xz A_z -> J_x; D_yz A_z -> J_y
+            {
+                const E* p = pl + 6 * M_PLANE;
+                const E f0 = p[0];
+                m_diff_sum<E, 1>(p, d, s);
+                m_diff_sum<E, M_WX>(p, e, t);
+                Bx[3] = m_dot3(c.c1y, e, Bx[3]);
+                By[3] = vsub(By[3], m_dot3(c.c1x, d));
+                const E pxy = vadd(m_dot3(c.c2x, s), m_dot3(c.c2y, t));
+                Pz[3] = vadd(vfma(c.c20all, f0, Pz[3]), pxy);
+                Jz[3] = vsub(vfma(c.nc20xy, f0, Jz[3]), pxy);
+#pragma unroll
+                for (int m = 1; m <= 3; m++) {
+                    M_SCAT(Pz, m, c.c2z[m - 1], c.c2z[m - 1], f0);
+                    M_SCAT(Jx, m, c.cmxz[m - 1], c.ncmxz[m - 1], d[m - 1]);
+                    M_SCAT(Jy, m, c.cmyz[m - 1], c.ncmyz[m - 1], e[m - 1]);
+                }
+            }
+
+            // ---- finalise level 0 ----
+            if (k >= 2 * R) {
+                const int z = zs + k - 2 * R;
+                const E b0 = vadd(Bx[0], c.bext[0]), b1 = vadd(By[0], c.bext[1]), b2 = vadd(Bz[0], c.bext[2]);
+                const E j0 = Jx[0], j1 = Jy[0], j2 = Jz[0];
+                const int u = k - 2 * R;
+                E* mb = (E*)(smem + M_OFF_MBOX + (u % M_ND) * M_MBOX_BYTES) + col;
+                mb[0] = vsub(vmul(j1, b2), vmul(j2, b1));
+                mb[M_COLS] = vsub(vmul(j2, b0), vmul(j0, b2));
+                mb[2 * M_COLS] = vsub(vmul(j0, b1), vmul(j1, b0));
+                __syncwarp();
+                if (lane == 0) m_bar_arrive(&mfull[pair * M_ND + u % M_ND]);
+                const E* pc = (const E*)(smem + ((k - R) % M_NP) * M_SLOT_BYTES) + cell_off;
+                const E ux = pc[M_PLANE], uy = pc[2 * M_PLANE], uz = pc[3 * M_PLANE];
+                const E ax = pc[4 * M_PLANE], ay = pc[5 * M_PLANE], az = pc[6 * M_PLANE];
+                // Eq. 3: u x B + eta lap A
+                const E r0 = vfma(c.eta, Px[0], vsub(vmul(uy, b2), vmul(uz, b1)));
+                const E r1 = vfma(c.eta, Py[0], vsub(vmul(uz, b0), vmul(ux, b2)));
+                const E r2 = vfma(c.eta, Pz[0], vsub(vmul(ux, b1), vmul(uy, b0)));
+                E o0 = ax, o1 = ay, o2 = az;
+                if (with_prev) {
+                    const E* pp = (const E*)(smem + M_OFF_PREV + (k % M_NPP) * M_PSLOT_BYTES) + 4 * M_COLS + col;
+                    o0 = vfma(c.rk_a, vsub(ax, pp[0]), o0);
+                    o1 = vfma(c.rk_a, vsub(ay, pp[M_COLS]), o1);
+                    o2 = vfma(c.rk_a, vsub(az, pp[2 * M_COLS]), o2);
+                }
+                o0 = vfma(c.rk_b, r0, o0);
+                o1 = vfma(c.rk_b, r1, o1);
+                o2 = vfma(c.rk_b, r2, o2);
+                if (valid) {
+                    const bool edge = edge_xy | (z < R) | (z >= L.nz - R);
+                    m_store<E>(a.out[4], L, x, y, z, o0, edge);
+                    m_store<E>(a.out[5], L, x, y, z, o1, edge);
+                    m_store<E>(a.out[6], L, x, y, z, o2, edge);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) m_bar_arrive(&done[k % M_NP]);
+#pragma unroll
+            for (int r = 0; r < 6; r++) {
+                Bx[r] = Bx[r + 1]; By[r] = By[r + 1]; Px[r] = Px[r + 1]; Py[r] = Py[r + 1]; Pz[r] = Pz[r + 1];
+                Jx[r] = Jx[r + 1]; Jy[r] = Jy[r + 1]; Jz[r] = Jz[r + 1];
+            }
+#pragma unroll
+            for (int r = 0; r < 3; r++) Bz[r] = Bz[r + 1];
+        }
+    }
+}
+
+}  // namespace ac
