@@ -62,7 +62,7 @@ constexpr int M_OFF_MBOX = M_OFF_PREV + M_NPP * M_PSLOT_BYTES;
 constexpr int M_OFF_ZTAB = M_OFF_MBOX + M_ND * M_MBOX_BYTES;
 constexpr int M_OFF_BARS = M_OFF_ZTAB + M_CZMAX * 2 * 8;
 constexpr int M_NBARS = 2 * M_NP + 4 * M_ND;
-constexpr int M_SMEM_BYTES = M_OFF_BARS + M_NBARS * 8 + 128;   // + slack for the 128-byte alignment of the base
+constexpr int M_SMEM_BYTES = M_OFF_BARS + M_NBARS * 8;
 static_assert(M_SLOT_BYTES % 128 == 0 && M_PSLOT_BYTES % 128 == 0, "TMA destinations must stay 128-byte aligned");
 static_assert(M_SMEM_BYTES <= 232448, "exceeds the 227 KB of shared memory a CTA may use");
 
@@ -179,19 +179,27 @@ __device__ __forceinline__ E m_mixxy(const E* p, const E (&cm)[3]) {
 // new value of a cell and its periodic ghost images; z images of packed pairs swap lanes
 template <typename E>
 __device__ __forceinline__ void m_store(E* __restrict__ o, const Layout& L, int x, int y, int z, E v, bool edge) {
-    o[L.idx(x, y, z)] = v;
+    E* p = o + L.idx(x, y, z);
+    *p = v;
     if (!edge) return;
-    int xs[2] = {x, x}, ys[2] = {y, y}, zs[3] = {z, z, z};
-    int cx = 1, cy = 1, cz = 1;
-    if (x < R) xs[cx++] = x + L.nx; else if (x >= L.nx - R) xs[cx++] = x - L.nx;
-    if (y < R) ys[cy++] = y + L.ny; else if (y >= L.ny - R) ys[cy++] = y - L.ny;
-    if (z < R) zs[cz++] = z + L.nz;
-    if (z >= L.nz - R) zs[cz++] = z - L.nz;      // both can hold when a packed grid has fewer than 6 planes
+    // element offsets of the periodic images along each axis (0 = none)
+    const ptrdiff_t ox = (x < R) ? L.nx : ((x >= L.nx - R) ? -L.nx : 0);
+    const ptrdiff_t oy = ((y < R) ? L.ny : ((y >= L.ny - R) ? -L.ny : 0)) * (ptrdiff_t)L.pitch;
+    const ptrdiff_t oz_up = (z < R) ? (ptrdiff_t)L.plane * L.nz : 0;
+    const ptrdiff_t oz_dn = (z >= L.nz - R) ? -(ptrdiff_t)L.plane * L.nz : 0;   // both can hold when a packed grid has fewer than 6 planes
+    if (ox) p[ox] = v;
+    if (oy) p[oy] = v;
+    if (ox && oy) p[ox + oy] = v;
     const E vs = vswap(v);
-    for (int k = 0; k < cz; k++)
-        for (int j = 0; j < cy; j++)
-            for (int i = 0; i < cx; i++)
-                if (i + j + k) o[L.idx(xs[i], ys[j], zs[k])] = k ? vs : v;
+#pragma unroll
+    for (int k = 0; k < 2; k++) {
+        const ptrdiff_t oz = k ? oz_dn : oz_up;
+        if (!oz) continue;
+        p[oz] = vs;
+        if (ox) p[oz + ox] = vs;
+        if (oy) p[oz + oy] = vs;
+        if (ox && oy) p[oz + ox + oy] = vs;
+    }
 }
 
 template <typename T>
@@ -199,8 +207,9 @@ __global__ void __launch_bounds__(M_THREADS, 1)
     substep_march_kernel(const __grid_constant__ MarchArgs<T> a, const __grid_constant__ CUtensorMap map_in,
                          const __grid_constant__ CUtensorMap map_prev) {
     using E = typename ElemOf<T>::E;
-    extern __shared__ unsigned char m_smem_raw[];
-    unsigned char* smem = (unsigned char*)(((uintptr_t)m_smem_raw + 127) & ~(uintptr_t)127);
+    // declared 1024-byte aligned and used in place: every pointer derived from it keeps the shared
+    // address space (LDS/STS); rounding the base through an integer made ptxas fall back to generic LD
+    extern __shared__ __align__(1024) unsigned char smem[];
     E* ztab = (E*)(smem + M_OFF_ZTAB);
     uint64_t* full = (uint64_t*)(smem + M_OFF_BARS);
     uint64_t* done = full + M_NP;
@@ -367,8 +376,7 @@ __global__ void __launch_bounds__(M_THREADS, 1)
                 rl = vfma(uy, g1, rl);
                 rl = vfma(uz, g2, rl);
                 rl = vneg(vadd(rl, divu));
-                const E rho_inv = vexpneg(lnrho);
-                // (j x B) from the A role of the same columns
+                // (j x B) / rho from the A role of the same columns
                 const int u = k - 2 * R;
                 m_bar_wait(&mfull[pair * M_ND + u % M_ND], (uint32_t)((u / M_ND) & 1));
                 const E* mb = (const E*)(smem + M_OFF_MBOX + (u % M_ND) * M_MBOX_BYTES) + col;
@@ -405,9 +413,9 @@ __global__ void __launch_bounds__(M_THREADS, 1)
                 E adv2 = vmul(ux, Gzx[0]);
                 adv2 = vfma(uy, Gzy[0], adv2);
                 adv2 = vfma(uz, Gzz[0], adv2);
-                E r0 = vfma(c.nu, vadd(Lx[0], sg0), vfma(jxb0, rho_inv, vsub(vmul(c.ncs2, g0), adv0)));
-                E r1 = vfma(c.nu, vadd(Ly[0], sg1), vfma(jxb1, rho_inv, vsub(vmul(c.ncs2, g1), adv1)));
-                E r2 = vfma(c.nu, vadd(Lz[0], sg2), vfma(jxb2, rho_inv, vsub(vmul(c.ncs2, g2), adv2)));
+                E r0 = vfma(c.nu, vadd(Lx[0], sg0), vadd(jxb0, vsub(vmul(c.ncs2, g0), adv0)));
+                E r1 = vfma(c.nu, vadd(Ly[0], sg1), vadd(jxb1, vsub(vmul(c.ncs2, g1), adv1)));
+                E r2 = vfma(c.nu, vadd(Lz[0], sg2), vadd(jxb2, vsub(vmul(c.ncs2, g2), adv2)));
                 if (a.has_forcing) {
                     r0 = vfma(c.fre[0], fc, vfma(c.nfim[0], fs, r0));
                     r1 = vfma(c.fre[1], fc, vfma(c.nfim[1], fs, r1));
@@ -527,13 +535,14 @@ __global__ void __launch_bounds__(M_THREADS, 1)
                 const E b0 = vadd(Bx[0], c.bext[0]), b1 = vadd(By[0], c.bext[1]), b2 = vadd(Bz[0], c.bext[2]);
                 const E j0 = Jx[0], j1 = Jy[0], j2 = Jz[0];
                 const int u = k - 2 * R;
+                const E* pc = (const E*)(smem + ((k - R) % M_NP) * M_SLOT_BYTES) + cell_off;
+                const E rho_inv = vexpneg(pc[0]);
                 E* mb = (E*)(smem + M_OFF_MBOX + (u % M_ND) * M_MBOX_BYTES) + col;
-                mb[0] = vsub(vmul(j1, b2), vmul(j2, b1));
-                mb[M_COLS] = vsub(vmul(j2, b0), vmul(j0, b2));
-                mb[2 * M_COLS] = vsub(vmul(j0, b1), vmul(j1, b0));
+                mb[0] = vmul(rho_inv, vsub(vmul(j1, b2), vmul(j2, b1)));
+                mb[M_COLS] = vmul(rho_inv, vsub(vmul(j2, b0), vmul(j0, b2)));
+                mb[2 * M_COLS] = vmul(rho_inv, vsub(vmul(j0, b1), vmul(j1, b0)));
                 __syncwarp();
                 if (lane == 0) m_bar_arrive(&mfull[pair * M_ND + u % M_ND]);
-                const E* pc = (const E*)(smem + ((k - R) % M_NP) * M_SLOT_BYTES) + cell_off;
                 const E ux = pc[M_PLANE], uy = pc[2 * M_PLANE], uz = pc[3 * M_PLANE];
                 const E ax = pc[4 * M_PLANE], ay = pc[5 * M_PLANE], az = pc[6 * M_PLANE];
                 // Eq. 3: u x B + eta lap A
