@@ -23,12 +23,15 @@
 // differences the first derivatives need anyway.  Quantities that enter the equations linearly
 // are accumulated already combined: L_i = lap u_i + 1/3 (grad div u)_i, lap A_i,
 // J_i = (grad div A - lap A)_i, B_i.  The cell at level 0 (plane p-3) is complete after plane p
-// has been scattered; it is then finalised: non-linear terms, forcing, 2N update, store (with the
-// periodic ghost images of boundary cells).
+// has been scattered; it is then finalised: non-linear terms, forcing, 2N update, store.  The
+// periodic ghost zones of the written buffer are refreshed by ghost_fill_kernel after the launch
+// (keeping the image stores inside this loop cost 15 % of the U role's issue slots and doubled
+// the loop's code size; profiles/r01b_march.md).
 //
 // Synchronisation: no block-wide barrier in the loop.  full[slot] (TMA transaction bytes) and
-// done[iteration] (one arrival per warp) mbarriers; lane 0 of warp 0 refills ring slots 3 planes
-// ahead once every warp has finished the iteration that last read them.  The A role hands
+// done[iteration] (one arrival per warp) mbarriers; the first lane of the A role (which runs ahead of
+// the U role) refills ring slots 3 planes ahead once every warp has finished the iteration that
+// last read them.  The A role hands
 // (j x B) to the U role of the same columns through a mailbox with one mbarrier per warp pair.
 //
 // Element type E (vec2.cuh): double, or f2 = two fp32 cells (z, z + nz/2) per element.
@@ -49,7 +52,7 @@ constexpr int M_WY = M_TY + 2 * R;       // 14
 constexpr int M_PLANE = M_WX * M_WY;     // elements per field per plane slot
 constexpr int M_NP = 8;                  // ring slots: planes p-3 .. p resident, p+1 .. p+3 in flight
 constexpr int M_NPP = 5;                 // previous-state ring slots
-constexpr int M_ND = 5;                  // mailbox depth
+constexpr int M_ND = 5;                  // mailbox depth: the A role runs at most 5 iterations ahead of the U role
 constexpr int M_LEAD = 3;                // planes issued ahead of the one being processed
 constexpr int M_CZMAX = 512;             // longest z chunk (bounds the z phase table in shared memory)
 constexpr int M_NF = 7;
@@ -111,12 +114,12 @@ __device__ __forceinline__ void m_bar_wait(uint64_t* bar, uint32_t parity) {
         "{\n"
         ".reg .pred p;\n"
         "MWAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
         "@p bra MDONE_%=;\n"
         "bra MWAIT_%=;\n"
         "MDONE_%=:\n"
         "}\n" ::"r"(m_smem_u32(bar)),
-        "r"(parity)
+        "r"(parity), "r"(0x4000u)      // suspend-time hint (ns): fewer polls of a role that runs ahead
         : "memory");
 }
 __device__ __forceinline__ void m_tma_load_4d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2,
@@ -176,29 +179,48 @@ __device__ __forceinline__ E m_mixxy(const E* p, const E (&cm)[3]) {
         acc[3 + (m)] = vfma((cup), (v), acc[3 + (m)]);        \
     } while (0)
 
-// new value of a cell and its periodic ghost images; z images of packed pairs swap lanes
+// S1, periodic ghost zones of one state buffer after a substep (the paper's "local boundary
+// transfer"; wrap of PAPER.md:111).  Every ghost cell copies its periodic source
+// cell, which is always an interior cell, so the order of the copies does not matter.  Blocks
+// [0, nb_rows * xb) serve the rows that are ghosts in y or z (whole rows, x ghosts included),
+// the remaining blocks the 2 x 3 x-ghost cells of the interior rows.  z images of packed fp32
+// pairs swap lanes (cell z - nz/2 of the pair below is cell z + nz/2 of the periodic domain).
+constexpr int M_GHOST_THREADS = 128;
 template <typename E>
-__device__ __forceinline__ void m_store(E* __restrict__ o, const Layout& L, int x, int y, int z, E v, bool edge) {
-    E* p = o + L.idx(x, y, z);
-    *p = v;
-    if (!edge) return;
-    // element offsets of the periodic images along each axis (0 = none)
-    const ptrdiff_t ox = (x < R) ? L.nx : ((x >= L.nx - R) ? -L.nx : 0);
-    const ptrdiff_t oy = ((y < R) ? L.ny : ((y >= L.ny - R) ? -L.ny : 0)) * (ptrdiff_t)L.pitch;
-    const ptrdiff_t oz_up = (z < R) ? (ptrdiff_t)L.plane * L.nz : 0;
-    const ptrdiff_t oz_dn = (z >= L.nz - R) ? -(ptrdiff_t)L.plane * L.nz : 0;   // both can hold when a packed grid has fewer than 6 planes
-    if (ox) p[ox] = v;
-    if (oy) p[oy] = v;
-    if (ox && oy) p[ox + oy] = v;
-    const E vs = vswap(v);
-#pragma unroll
-    for (int k = 0; k < 2; k++) {
-        const ptrdiff_t oz = k ? oz_dn : oz_up;
-        if (!oz) continue;
-        p[oz] = vs;
-        if (ox) p[oz + ox] = vs;
-        if (oy) p[oz + oy] = vs;
-        if (ox && oy) p[oz + ox + oy] = vs;
+__global__ void __launch_bounds__(M_GHOST_THREADS) ghost_fill_kernel(E* __restrict__ base, Layout L, int nb_rows, int xb) {
+    E* __restrict__ f = base + (size_t)blockIdx.y * L.field;
+    const long b = blockIdx.x;
+    const long nb = (long)nb_rows * xb;
+    if (b < nb) {
+        const int row = (int)(b / xb);
+        const int x = (int)(b % xb) * M_GHOST_THREADS + (int)threadIdx.x - R;
+        if (x >= L.nx + R) return;
+        int y, z;
+        if (row < 2 * R * L.my) {            // the 6 ghost planes, all rows
+            const int zi = row / L.my;
+            z = zi < R ? zi - R : L.nz + zi - R;
+            y = row % L.my - R;
+        } else {                             // the 6 ghost rows of every interior plane
+            const int r2 = row - 2 * R * L.my;
+            const int yi = r2 % (2 * R);
+            z = r2 / (2 * R);
+            y = yi < R ? yi - R : L.ny + yi - R;
+        }
+        const int xs = x < 0 ? x + L.nx : (x >= L.nx ? x - L.nx : x);
+        const int ys = y < 0 ? y + L.ny : (y >= L.ny ? y - L.ny : y);
+        const int zs = z < 0 ? z + L.nz : (z >= L.nz ? z - L.nz : z);
+        E v = f[L.idx(xs, ys, zs)];
+        if (zs != z) v = vswap(v);
+        f[L.idx(x, y, z)] = v;
+    } else {
+        const long t = (b - nb) * M_GHOST_THREADS + threadIdx.x;
+        const int j = (int)(t & 7);
+        const long r = t >> 3;
+        if (j >= 2 * R || r >= (long)L.ny * L.nz) return;
+        const int y = (int)(r % L.ny), z = (int)(r / L.ny);
+        const int x = j < R ? j - R : L.nx + j - R;
+        const int xs = j < R ? x + L.nx : x - L.nx;
+        f[L.idx(x, y, z)] = f[L.idx(xs, y, z)];
     }
 }
 
@@ -229,7 +251,6 @@ __global__ void __launch_bounds__(M_THREADS, 1)
     const int niter = ze - zs + 2 * R;      // planes zs-3 .. ze+2
     const int x = x0 + tx, y = y0 + ty;
     const bool valid = (x < L.nx) && (y < L.ny);
-    const bool edge_xy = (x < R) | (x >= L.nx - R) | (y < R) | (y >= L.ny - R);
     const bool with_prev = a.substep != 0;
 
     if (tid == 0) {
@@ -262,7 +283,7 @@ __global__ void __launch_bounds__(M_THREADS, 1)
             m_tma_load_4d(smem + M_OFF_PREV + (k % M_NPP) * M_PSLOT_BYTES, &map_prev, &full[slot], x0 + L.gx, y0 + R,
                           zs + k - R, 0);
     };
-    if (tid == 0)
+    if (tid == M_COLS)
         for (int k = 0; k < M_LEAD && k < niter; k++) issue(k);
 
     const int cell_off = (ty + R) * M_WX + tx + M_HX;
@@ -278,24 +299,25 @@ __global__ void __launch_bounds__(M_THREADS, 1)
 
     if (role == 0) {
         // ======================================= U role ========================================
-        E gz[7], Gxz[7], Gyz[7], Gzz[7], Lx[7], Ly[7], Lz[7];     // z-coupled accumulators, levels 0..6
-        E gx[4], gy[4], Gxx[4], Gxy[4], Gyx[4], Gyy[4], Gzx[4], Gzy[4];   // in-plane first derivatives, levels 0..3
+        E Gxz[7], Gyz[7], Gzz[7], Lx[7], Ly[7], Lz[7];            // z-coupled accumulators, levels 0..6
+        E Gxx[4], Gxy[4], Gyx[4], Gyy[4], Gzx[4], Gzy[4];         // in-plane first derivatives, levels 0..3
+        E gz[7], gx[4], gy[4];
 #pragma unroll
-        for (int r = 0; r < 7; r++) gz[r] = Gxz[r] = Gyz[r] = Gzz[r] = Lx[r] = Ly[r] = Lz[r] = vzero<E>();
+        for (int r = 0; r < 7; r++) gz[r] = vzero<E>();
 #pragma unroll
-        for (int r = 0; r < 4; r++) gx[r] = gy[r] = Gxx[r] = Gxy[r] = Gyx[r] = Gyy[r] = Gzx[r] = Gzy[r] = vzero<E>();
+        for (int r = 0; r < 4; r++) gx[r] = gy[r] = vzero<E>();
+#pragma unroll
+        for (int r = 0; r < 7; r++) Gxz[r] = Gyz[r] = Gzz[r] = Lx[r] = Ly[r] = Lz[r] = vzero<E>();
+#pragma unroll
+        for (int r = 0; r < 4; r++) Gxx[r] = Gxy[r] = Gyx[r] = Gyy[r] = Gzx[r] = Gzy[r] = vzero<E>();
 
         for (int k = 0; k < niter; k++) {
-            if (tid == 0 && k + M_LEAD < niter) {
-                if (k >= 2) m_bar_wait(&done[(k - 2) % M_NP], (uint32_t)(((k - 2) / M_NP) & 1));
-                issue(k + M_LEAD);
-            }
             m_bar_wait(&full[k % M_NP], (uint32_t)((k / M_NP) & 1));
             const E* pl = (const E*)(smem + (k % M_NP) * M_SLOT_BYTES) + cell_off;
 
-            gz[6] = Gxz[6] = Gyz[6] = Gzz[6] = Lx[6] = Ly[6] = Lz[6] = vzero<E>();
+            Gxz[6] = Gyz[6] = Gzz[6] = Lx[6] = Ly[6] = Lz[6] = vzero<E>();
             E d[3], s[3], e[3], t[3];
-            // ---- ln rho ----
+            gz[6] = vzero<E>();
             {
                 const E* p = pl;
                 const E f0 = p[0];
@@ -369,18 +391,18 @@ __global__ void __launch_bounds__(M_THREADS, 1)
                 const int z = zs + k - 2 * R;
                 const E* pc = (const E*)(smem + ((k - R) % M_NP) * M_SLOT_BYTES) + cell_off;
                 const E lnrho = pc[0], ux = pc[M_PLANE], uy = pc[2 * M_PLANE], uz = pc[3 * M_PLANE];
-                const E g0 = gx[0], g1 = gy[0], g2 = gz[0];
                 const E divu = vadd(vadd(Gxx[0], Gyy[0]), Gzz[0]);
+                // (j x B) / rho and grad ln rho from the A role of the same columns
+                const int u = k - 2 * R;
+                m_bar_wait(&mfull[pair * M_ND + u % M_ND], (uint32_t)((u / M_ND) & 1));
+                const E* mb = (const E*)(smem + M_OFF_MBOX + (u % M_ND) * M_MBOX_BYTES) + col;
+                const E jxb0 = mb[0], jxb1 = mb[M_COLS], jxb2 = mb[2 * M_COLS];
+                const E g0 = gx[0], g1 = gy[0], g2 = gz[0];
                 // Eq. 1
                 E rl = vmul(ux, g0);
                 rl = vfma(uy, g1, rl);
                 rl = vfma(uz, g2, rl);
                 rl = vneg(vadd(rl, divu));
-                // (j x B) / rho from the A role of the same columns
-                const int u = k - 2 * R;
-                m_bar_wait(&mfull[pair * M_ND + u % M_ND], (uint32_t)((u / M_ND) & 1));
-                const E* mb = (const E*)(smem + M_OFF_MBOX + (u % M_ND) * M_MBOX_BYTES) + col;
-                const E jxb0 = mb[0], jxb1 = mb[M_COLS], jxb2 = mb[2 * M_COLS];
                 // forcing Eq. 4: f_i = re_i cos(theta) - im_i sin(theta)
                 E fc = vzero<E>(), fs = vzero<E>();
                 if (a.has_forcing) {
@@ -434,12 +456,12 @@ __global__ void __launch_bounds__(M_THREADS, 1)
                 o1 = vfma(c.rk_b, r0, o1);
                 o2 = vfma(c.rk_b, r1, o2);
                 o3 = vfma(c.rk_b, r2, o3);
+                const size_t ci = L.idx(x, y, z);
                 if (valid) {
-                    const bool edge = edge_xy | (z < R) | (z >= L.nz - R);
-                    m_store<E>(a.out[0], L, x, y, z, o0, edge);
-                    m_store<E>(a.out[1], L, x, y, z, o1, edge);
-                    m_store<E>(a.out[2], L, x, y, z, o2, edge);
-                    m_store<E>(a.out[3], L, x, y, z, o3, edge);
+                    a.out[0][ci] = o0;
+                    a.out[1][ci] = o1;
+                    a.out[2][ci] = o2;
+                    a.out[3][ci] = o3;
                 }
             }
             __syncwarp();
@@ -447,14 +469,18 @@ __global__ void __launch_bounds__(M_THREADS, 1)
             // next plane: every pending level moves one step closer to completion
 #pragma unroll
             for (int r = 0; r < 6; r++) {
-                gz[r] = gz[r + 1]; Gxz[r] = Gxz[r + 1]; Gyz[r] = Gyz[r + 1]; Gzz[r] = Gzz[r + 1];
+                Gxz[r] = Gxz[r + 1]; Gyz[r] = Gyz[r + 1]; Gzz[r] = Gzz[r + 1];
                 Lx[r] = Lx[r + 1]; Ly[r] = Ly[r + 1]; Lz[r] = Lz[r + 1];
             }
 #pragma unroll
             for (int r = 0; r < 3; r++) {
-                gx[r] = gx[r + 1]; gy[r] = gy[r + 1]; Gxx[r] = Gxx[r + 1]; Gxy[r] = Gxy[r + 1];
+                Gxx[r] = Gxx[r + 1]; Gxy[r] = Gxy[r + 1];
                 Gyx[r] = Gyx[r + 1]; Gyy[r] = Gyy[r + 1]; Gzx[r] = Gzx[r + 1]; Gzy[r] = Gzy[r + 1];
             }
+#pragma unroll
+            for (int r = 0; r < 6; r++) gz[r] = gz[r + 1];
+#pragma unroll
+            for (int r = 0; r < 3; r++) { gx[r] = gx[r + 1]; gy[r] = gy[r + 1]; }
         }
     } else {
         // ======================================= A role ========================================
@@ -466,6 +492,12 @@ __global__ void __launch_bounds__(M_THREADS, 1)
         for (int r = 0; r < 4; r++) Bz[r] = vzero<E>();
 
         for (int k = 0; k < niter; k++) {
+            // this role runs ahead of the U role, so its first lane also feeds the ring: plane
+            // k + LEAD reuses the slot that every warp has released after iteration k - 2
+            if (tid == M_COLS && k + M_LEAD < niter) {
+                if (k >= 2) m_bar_wait(&done[(k - 2) % M_NP], (uint32_t)(((k - 2) / M_NP) & 1));
+                issue(k + M_LEAD);
+            }
             m_bar_wait(&full[k % M_NP], (uint32_t)((k / M_NP) & 1));
             const E* pl = (const E*)(smem + (k % M_NP) * M_SLOT_BYTES) + cell_off;
 
@@ -559,11 +591,11 @@ __global__ void __launch_bounds__(M_THREADS, 1)
                 o0 = vfma(c.rk_b, r0, o0);
                 o1 = vfma(c.rk_b, r1, o1);
                 o2 = vfma(c.rk_b, r2, o2);
+                const size_t ci = L.idx(x, y, z);
                 if (valid) {
-                    const bool edge = edge_xy | (z < R) | (z >= L.nz - R);
-                    m_store<E>(a.out[4], L, x, y, z, o0, edge);
-                    m_store<E>(a.out[5], L, x, y, z, o1, edge);
-                    m_store<E>(a.out[6], L, x, y, z, o2, edge);
+                    a.out[4][ci] = o0;
+                    a.out[5][ci] = o1;
+                    a.out[6][ci] = o2;
                 }
             }
             __syncwarp();
