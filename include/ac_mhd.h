@@ -105,7 +105,16 @@ int ac_load_state(ac_ctx* ctx, const void* const fields[AC_NFIELDS], int src_on_
  * stream before returning.  Device destinations: asynchronous on the stream. */
 int ac_store_state(ac_ctx* ctx, void* const fields[AC_NFIELDS], int dst_on_device);
 
-/* One full RK3 time step = 3 fused substep kernels (S1-S8 of DESIGN.md), asynchronous.
+/* The same for ONE field (q = AC_LNRHO .. AC_AZ order: ln rho, ux, uy, uz, ax, ay, az), so that a
+ * caller can stream a state that is too large to hold twice (1024^3 fp64: 8.6 GB per field next
+ * to the 122.6 GB workspace).  ac_load_field writes field q of the current state; the context
+ * counts as loaded once all 7 fields have been written since ac_init / the last ac_load_state.
+ * A host source is staged in the idle state buffer.  Errors: AC_EINVAL, AC_ESTATE (store), AC_ECUDA. */
+int ac_load_field(ac_ctx* ctx, int q, const void* field, int src_on_device);
+int ac_store_field(ac_ctx* ctx, int q, void* field, int dst_on_device);
+
+/* One full RK3 time step = 3 fused substep kernels (S1-S8 of DESIGN.md), each followed by the
+ * ghost-zone kernel (S1) in the default variant, asynchronous.
  * forcing == NULL: no forcing.  The same forcing parameters are used in all 3 substeps (G8).
  * Errors: AC_EINVAL (dt <= 0 or non-finite), AC_ESTATE, AC_ECUDA. */
 int ac_step(ac_ctx* ctx, double dt, const ac_forcing* forcing);

@@ -15,7 +15,8 @@ LIB_PATH = os.path.join(_HERE, "libac_mhd.so")
 AC_F32, AC_F64 = 0, 1
 NFIELDS = 7
 EXPORTS = (
-    "ac_workspace_bytes", "ac_init", "ac_load_state", "ac_store_state", "ac_step", "ac_reduce",
+    "ac_workspace_bytes", "ac_init", "ac_load_state", "ac_store_state", "ac_load_field", "ac_store_field", "ac_step",
+    "ac_reduce",
     "ac_forcing_from_draws", "ac_forcing_params", "ac_make_forcing", "ac_set_bext", "ac_set_cfl", "ac_set_variant",
     "ac_launch_count", "ac_free", "ac_strerror", "ac_version",
 )
@@ -75,6 +76,8 @@ def load_library():
     L.ac_init.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(AcGrid), i32, dbl, dbl, dbl, dbl, dbl, vp, vp]
     L.ac_load_state.argtypes = [vp, ctypes.POINTER(vp), i32]
     L.ac_store_state.argtypes = [vp, ctypes.POINTER(vp), i32]
+    L.ac_load_field.argtypes = [vp, i32, vp, i32]
+    L.ac_store_field.argtypes = [vp, i32, vp, i32]
     L.ac_step.argtypes = [vp, dbl, ctypes.POINTER(AcForcing)]
     L.ac_reduce.argtypes = [vp, ctypes.POINTER(AcDiag)]
     L.ac_forcing_from_draws.argtypes = [vp, dbl, dbl, dbl, dbl, dbl, ctypes.POINTER(AcForcing)]
@@ -91,7 +94,7 @@ def load_library():
     L.ac_strerror.argtypes = [i32]
     L.ac_strerror.restype = ctypes.c_char_p
     L.ac_version.restype = ctypes.c_char_p
-    for name in ("ac_init", "ac_load_state", "ac_store_state", "ac_step", "ac_reduce", "ac_forcing_from_draws",
+    for name in ("ac_init", "ac_load_state", "ac_store_state", "ac_load_field", "ac_store_field", "ac_step", "ac_reduce", "ac_forcing_from_draws",
                  "ac_forcing_params", "ac_make_forcing", "ac_set_bext", "ac_set_cfl", "ac_set_variant"):
         getattr(L, name).restype = i32
     _lib = L
@@ -197,6 +200,25 @@ class Context:
             ptrs = [out[q].data_ptr() for q in range(NFIELDS)]
             on_dev = 1 if out.is_cuda else 0
         _check(self._lib.ac_store_state(self._ctx, self._ptr_array(ptrs), on_dev), "ac_store_state")
+        return out
+
+    def _field_ptr(self, arr):
+        if isinstance(arr, np.ndarray):
+            assert arr.dtype == self.np_dtype and arr.flags["C_CONTIGUOUS"] and arr.shape == self.shape
+            return arr.ctypes.data, 0
+        assert arr.dtype == self.torch_dtype and arr.is_contiguous() and tuple(arr.shape) == self.shape
+        return arr.data_ptr(), (1 if arr.is_cuda else 0)
+
+    def ac_load_field(self, q, field):
+        """field: numpy (nz, ny, nx) or torch tensor (host or device) of the context's dtype."""
+        ptr, on_dev = self._field_ptr(field)
+        _check(self._lib.ac_load_field(self._ctx, int(q), ctypes.c_void_p(ptr), on_dev), "ac_load_field")
+        if not on_dev:
+            self.synchronize()
+
+    def ac_store_field(self, q, out):
+        ptr, on_dev = self._field_ptr(out)
+        _check(self._lib.ac_store_field(self._ctx, int(q), ctypes.c_void_p(ptr), on_dev), "ac_store_field")
         return out
 
     def ac_step(self, dt, forcing=None):

@@ -147,6 +147,7 @@ struct ac_ctx {
     cudaStream_t stream;
     int cur;  // which of the two state buffers holds the current state
     bool loaded;
+    unsigned loaded_mask;  // fields written since the last ac_load_state / configure (ac_load_field)
     long long launches;
     ac::RedVals* host_result;  // pinned
     CUtensorMap map_in[2];     // TMA maps of the two state buffers: tile + halo boxes
@@ -173,53 +174,47 @@ void fill_coeffs(const ac_ctx* ctx, ac::Coeffs<T>& c) {
         for (int m = 0; m < 3; m++) c.cm[p][m] = (T)(WM[m] / (h[pa[p]] * h[pb[p]]));
 }
 
+// one field: dense caller layout -> padded device layout of state buffer `buf` (ghost zones by periodic wrap)
 template <typename T>
-int load_state_t(ac_ctx* ctx, const void* const fields[AC_NFIELDS], int src_on_device) {
+int load_field_t(ac_ctx* ctx, int buf, int q, const void* field, int src_on_device) {
     const ac::Layout& L = ctx->L;
     const ac_grid& g = ctx->grid;
     const size_t dense_bytes = (size_t)g.nx * g.ny * g.nz * sizeof(T);
     dim3 blk(64, 4, 1);
     dim3 grd((L.nx + 2 * ac::R + blk.x - 1) / blk.x, (L.ny + 2 * ac::R + blk.y - 1) / blk.y, L.nz + 2 * ac::R);
-    for (int q = 0; q < AC_NFIELDS; q++) {
-        const T* src;
-        if (src_on_device) {
-            src = (const T*)fields[q];
-        } else {
-            // stage the dense field in the second state buffer, whose contents are dead between steps
-            T* stage = (T*)ctx->field_ptr(1, q);
-            AC_CUDA(cudaMemcpyAsync(stage, fields[q], dense_bytes, cudaMemcpyHostToDevice, ctx->stream));
-            src = stage;
-        }
-        if (ctx->packed)
-            ac::pack_pairs_kernel<<<grd, blk, 0, ctx->stream>>>((const float*)src, (float2*)ctx->field_ptr(0, q), L, g.nz);
-        else
-            ac::pack_kernel<T><<<grd, blk, 0, ctx->stream>>>(src, (T*)ctx->field_ptr(0, q), L);
-        ctx->launches++;
+    const T* src;
+    if (src_on_device) {
+        src = (const T*)field;
+    } else {
+        // stage the dense field in the other state buffer, whose contents are dead between steps
+        T* stage = (T*)ctx->field_ptr(1 - buf, q);
+        AC_CUDA(cudaMemcpyAsync(stage, field, dense_bytes, cudaMemcpyHostToDevice, ctx->stream));
+        src = stage;
     }
+    if (ctx->packed)
+        ac::pack_pairs_kernel<<<grd, blk, 0, ctx->stream>>>((const float*)src, (float2*)ctx->field_ptr(buf, q), L, g.nz);
+    else
+        ac::pack_kernel<T><<<grd, blk, 0, ctx->stream>>>(src, (T*)ctx->field_ptr(buf, q), L);
+    ctx->launches++;
     AC_CUDA(cudaGetLastError());
-    ctx->cur = 0;
-    ctx->loaded = true;
     return AC_OK;
 }
 
 template <typename T>
-int store_state_t(ac_ctx* ctx, void* const fields[AC_NFIELDS], int dst_on_device) {
+int store_field_t(ac_ctx* ctx, int q, void* field, int dst_on_device) {
     const ac::Layout& L = ctx->L;
     const ac_grid& g = ctx->grid;
     const size_t dense_bytes = (size_t)g.nx * g.ny * g.nz * sizeof(T);
     dim3 blk(64, 4, 1);
     dim3 grd((L.nx + blk.x - 1) / blk.x, (L.ny + blk.y - 1) / blk.y, L.nz);
-    for (int q = 0; q < AC_NFIELDS; q++) {
-        T* dst = dst_on_device ? (T*)fields[q] : (T*)ctx->field_ptr(1 - ctx->cur, q);
-        if (ctx->packed)
-            ac::unpack_pairs_kernel<<<grd, blk, 0, ctx->stream>>>((const float2*)ctx->field_ptr(ctx->cur, q), (float*)dst, L);
-        else
-            ac::unpack_kernel<T><<<grd, blk, 0, ctx->stream>>>((const T*)ctx->field_ptr(ctx->cur, q), dst, L);
-        if (!dst_on_device) AC_CUDA(cudaMemcpyAsync(fields[q], dst, dense_bytes, cudaMemcpyDeviceToHost, ctx->stream));
-        ctx->launches++;
-    }
+    T* dst = dst_on_device ? (T*)field : (T*)ctx->field_ptr(1 - ctx->cur, q);
+    if (ctx->packed)
+        ac::unpack_pairs_kernel<<<grd, blk, 0, ctx->stream>>>((const float2*)ctx->field_ptr(ctx->cur, q), (float*)dst, L);
+    else
+        ac::unpack_kernel<T><<<grd, blk, 0, ctx->stream>>>((const T*)ctx->field_ptr(ctx->cur, q), dst, L);
+    ctx->launches++;
+    if (!dst_on_device) AC_CUDA(cudaMemcpyAsync(field, dst, dense_bytes, cudaMemcpyDeviceToHost, ctx->stream));
     AC_CUDA(cudaGetLastError());
-    if (!dst_on_device) AC_CUDA(cudaStreamSynchronize(ctx->stream));
     return AC_OK;
 }
 
@@ -454,6 +449,7 @@ int configure(ac_ctx* ctx) {
     ctx->L = layout_for(g, ctx->dtype, ctx->packed);
     ctx->cv = carve(ctx->L, store_elem_size(ctx->dtype, ctx->packed), elem_size(ctx->dtype), g->nz);
     ctx->loaded = false;
+    ctx->loaded_mask = 0;
     ctx->cur = 0;
     if (!ctx->march) return AC_OK;
     for (int b = 0; b < 2; b++) {
@@ -570,8 +566,24 @@ int ac_load_state(ac_ctx* ctx, const void* const fields[AC_NFIELDS], int src_on_
     if (!ctx || !fields) return AC_EINVAL;
     for (int q = 0; q < AC_NFIELDS; q++)
         if (!fields[q]) return AC_EINVAL;
-    return ctx->dtype == AC_F64 ? load_state_t<double>(ctx, fields, src_on_device)
-                                : load_state_t<float>(ctx, fields, src_on_device);
+    ctx->cur = 0;
+    ctx->loaded = false;
+    ctx->loaded_mask = 0;
+    for (int q = 0; q < AC_NFIELDS; q++) {
+        const int rc = ac_load_field(ctx, q, fields[q], src_on_device);
+        if (rc != AC_OK) return rc;
+    }
+    return AC_OK;
+}
+
+int ac_load_field(ac_ctx* ctx, int q, const void* field, int src_on_device) {
+    if (!ctx || !field || q < 0 || q >= AC_NFIELDS) return AC_EINVAL;
+    const int rc = ctx->dtype == AC_F64 ? load_field_t<double>(ctx, ctx->cur, q, field, src_on_device)
+                                        : load_field_t<float>(ctx, ctx->cur, q, field, src_on_device);
+    if (rc != AC_OK) return rc;
+    ctx->loaded_mask |= 1u << q;
+    if (ctx->loaded_mask == (1u << AC_NFIELDS) - 1u) ctx->loaded = true;
+    return AC_OK;
 }
 
 int ac_store_state(ac_ctx* ctx, void* const fields[AC_NFIELDS], int dst_on_device) {
@@ -579,8 +591,23 @@ int ac_store_state(ac_ctx* ctx, void* const fields[AC_NFIELDS], int dst_on_devic
     for (int q = 0; q < AC_NFIELDS; q++)
         if (!fields[q]) return AC_EINVAL;
     if (!ctx->loaded) return AC_ESTATE;
-    return ctx->dtype == AC_F64 ? store_state_t<double>(ctx, fields, dst_on_device)
-                                : store_state_t<float>(ctx, fields, dst_on_device);
+    for (int q = 0; q < AC_NFIELDS; q++) {
+        const int rc = ctx->dtype == AC_F64 ? store_field_t<double>(ctx, q, fields[q], dst_on_device)
+                                            : store_field_t<float>(ctx, q, fields[q], dst_on_device);
+        if (rc != AC_OK) return rc;
+    }
+    if (!dst_on_device) AC_CUDA(cudaStreamSynchronize(ctx->stream));
+    return AC_OK;
+}
+
+int ac_store_field(ac_ctx* ctx, int q, void* field, int dst_on_device) {
+    if (!ctx || !field || q < 0 || q >= AC_NFIELDS) return AC_EINVAL;
+    if (!ctx->loaded) return AC_ESTATE;
+    const int rc = ctx->dtype == AC_F64 ? store_field_t<double>(ctx, q, field, dst_on_device)
+                                        : store_field_t<float>(ctx, q, field, dst_on_device);
+    if (rc != AC_OK) return rc;
+    if (!dst_on_device) AC_CUDA(cudaStreamSynchronize(ctx->stream));
+    return AC_OK;
 }
 
 int ac_step(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
