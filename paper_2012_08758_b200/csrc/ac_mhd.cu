@@ -365,12 +365,18 @@ int reduce_t(ac_ctx* ctx, ac_diag* out) {
     for (int q = 0; q < AC_NFIELDS; q++) a.in[q] = ctx->field_ptr(ctx->cur, q);
     a.partial = (ac::RedVals*)(ctx->ws + ctx->cv.partial_off);
     ac::RedVals* result = (ac::RedVals*)(ctx->ws + ctx->cv.result_off);
-    const long rows = (long)L.ny * L.nz;
-    const int blocks = (int)std::min<long>(rows, RED_BLOCKS);
-    if (ctx->packed)
-        ac::reduce_stage1_kernel<T, 2><<<blocks, 256, 0, ctx->stream>>>(a);
-    else
-        ac::reduce_stage1_kernel<T, 1><<<blocks, 256, 0, ctx->stream>>>(a);
+    const int tiles_x = (L.nx + ac::RED_TX - 1) / ac::RED_TX, tiles_y = (L.ny + ac::RED_TY - 1) / ac::RED_TY;
+    const int nchunks = (L.nz + ac::RED_CZ - 1) / ac::RED_CZ;
+    const int blocks = (int)std::min<long>((long)tiles_x * tiles_y * nchunks, RED_BLOCKS);
+    if (ctx->packed) {
+        const int sm = ac::red_smem_bytes<T, 2>();
+        AC_CUDA(cudaFuncSetAttribute(ac::reduce_stage1_kernel<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
+        ac::reduce_stage1_kernel<T, 2><<<blocks, ac::RED_THREADS, sm, ctx->stream>>>(a, tiles_x, tiles_y, nchunks);
+    } else {
+        const int sm = ac::red_smem_bytes<T, 1>();
+        AC_CUDA(cudaFuncSetAttribute(ac::reduce_stage1_kernel<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
+        ac::reduce_stage1_kernel<T, 1><<<blocks, ac::RED_THREADS, sm, ctx->stream>>>(a, tiles_x, tiles_y, nchunks);
+    }
     ac::reduce_stage2_kernel<<<1, 256, 0, ctx->stream>>>(a.partial, blocks, result);
     ctx->launches += 2;
     AC_CUDA(cudaGetLastError());

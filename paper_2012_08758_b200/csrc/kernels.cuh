@@ -243,65 +243,118 @@ __device__ __forceinline__ void red_load(const void* base, size_t i, T (&v)[LANE
     }
 }
 
-// stage 1: each block owns a fixed set of (y, z) rows; one partial per block.  LANES = 2: packed fp32 pairs.
+// stage 1: a block of 32 x 8 threads takes (x, y) tiles of one z chunk at a time (fixed round-robin
+// assignment, so the result is deterministic) and marches along z.  Per cell it loads the 7 centre
+// values and the 24 in-plane neighbours that curl A needs (d_x, d_y of A_z, d_x A_y, d_y A_x), all
+// from the plane it is visiting, so the neighbour loads hit the lines its own block has just
+// brought into L1.  The z derivatives of A_x, A_y come from a 7-plane history and the in-plane
+// parts of B wait 3 planes; both live in thread-private columns of shared memory (ring-indexed, no
+// barrier: a thread only reads what it wrote) so that the registers stay free for the 31 loads in
+// flight.  31 loads per cell instead of 43.  One partial per block.
+// LANES = 2: packed fp32 pairs (ghost planes hold lane-swapped pairs, so the history needs no care).
+constexpr int RED_TX = 32, RED_TY = 8, RED_THREADS = RED_TX * RED_TY, RED_CZ = 32;
 template <typename T, int LANES>
-__global__ void __launch_bounds__(256) reduce_stage1_kernel(const __grid_constant__ ReduceArgs<T> a) {
+constexpr int red_smem_bytes() {
+    return (2 * 7 + 3 * 4) * RED_THREADS * LANES * (int)sizeof(T);
+}
+template <typename T, int LANES>
+__global__ void __launch_bounds__(RED_THREADS, 2) reduce_stage1_kernel(const __grid_constant__ ReduceArgs<T> a, int tiles_x,
+                                                                       int tiles_y, int nchunks) {
+    extern __shared__ __align__(16) unsigned char red_smem[];
+    typedef T Col[RED_THREADS][LANES];
+    Col* hax = (Col*)red_smem;          // [7]  A_x of planes p-6 .. p, slot = plane mod 7
+    Col* hay = hax + 7;                 // [7]
+    Col* pbx = hay + 7;                 // [4]  d_y A_z of planes p-3 .. p, slot = plane mod 4
+    Col* pby = pbx + 4;                 // [4]  d_x A_z
+    Col* pbz = pby + 4;                 // [4]  B_z
     const Layout& L = a.L;
     RedVals acc = red_identity();
     const long pitch = L.pitch, plane = (long)L.plane;
-    const long rows = (long)L.ny * L.nz;
-    for (long row = blockIdx.x; row < rows; row += gridDim.x) {
-        const int y = (int)(row % L.ny), z = (int)(row / L.ny);
-        for (int x = threadIdx.x; x < L.nx; x += blockDim.x) {
-            const size_t c0 = L.idx(x, y, z);
-            T ux[LANES], uy[LANES], uz[LANES], l[LANES], ax[LANES], ay[LANES], az[LANES];
-            red_load<T, LANES>(a.in[UX], c0, ux);
-            red_load<T, LANES>(a.in[UY], c0, uy);
-            red_load<T, LANES>(a.in[UZ], c0, uz);
-            red_load<T, LANES>(a.in[LNRHO], c0, l);
-            red_load<T, LANES>(a.in[AX], c0, ax);
-            red_load<T, LANES>(a.in[AY], c0, ay);
-            red_load<T, LANES>(a.in[AZ], c0, az);
-            // first derivative of field q along an axis with element stride `stride`
-            auto d = [&](int q, long stride, int axis, T (&r)[LANES]) {
-                T p1[LANES], m1[LANES], p2[LANES], m2[LANES], p3[LANES], m3[LANES];
-                red_load<T, LANES>(a.in[q], c0 + stride, p1);
-                red_load<T, LANES>(a.in[q], c0 - stride, m1);
-                red_load<T, LANES>(a.in[q], c0 + 2 * stride, p2);
-                red_load<T, LANES>(a.in[q], c0 - 2 * stride, m2);
-                red_load<T, LANES>(a.in[q], c0 + 3 * stride, p3);
-                red_load<T, LANES>(a.in[q], c0 - 3 * stride, m3);
+    const long nwork = (long)tiles_x * tiles_y * nchunks;
+    const int tid = threadIdx.x;
+    const int tx = tid & (RED_TX - 1), ty = tid / RED_TX;
+    for (long w = blockIdx.x; w < nwork; w += gridDim.x) {
+        const int x = (int)(w % tiles_x) * RED_TX + tx;
+        const int y = (int)((w / tiles_x) % tiles_y) * RED_TY + ty;
+        const int zs = (int)(w / ((long)tiles_x * tiles_y)) * RED_CZ;
+        const int ze = min(zs + RED_CZ, L.nz);
+        if (x >= L.nx || y >= L.ny) continue;
+        size_t c0 = L.idx(x, y, zs - R);
+        int s7 = 0, s4 = 0;                                  // ring slots of the plane being visited
+#pragma unroll 1
+        for (int p = zs - R; p < ze + R; p++, c0 += plane) {
+            T vax[LANES], vay[LANES];
+            red_load<T, LANES>(a.in[AX], c0, vax);
+            red_load<T, LANES>(a.in[AY], c0, vay);
+            if (p >= zs && p < ze) {
+                T ux[LANES], uy[LANES], uz[LANES], l[LANES], az[LANES];
+                T n[4][6][LANES];                            // the 24 in-plane neighbours
+                red_load<T, LANES>(a.in[UX], c0, ux);
+                red_load<T, LANES>(a.in[UY], c0, uy);
+                red_load<T, LANES>(a.in[UZ], c0, uz);
+                red_load<T, LANES>(a.in[LNRHO], c0, l);
+                red_load<T, LANES>(a.in[AZ], c0, az);
+                const int fq[4] = {AZ, AZ, AY, AX};
+                const long fs[4] = {pitch, 1, 1, pitch};
+#pragma unroll
+                for (int k = 0; k < 4; k++)
+#pragma unroll
+                    for (int m = 1; m <= 3; m++) {
+                        red_load<T, LANES>(a.in[fq[k]], c0 + m * fs[k], n[k][2 * (m - 1)]);
+                        red_load<T, LANES>(a.in[fq[k]], c0 - m * fs[k], n[k][2 * (m - 1) + 1]);
+                    }
+                const int fa[4] = {1, 0, 0, 1};              // axis of the derivative
+                T dd[4][LANES];                              // d_y A_z, d_x A_z, d_x A_y, d_y A_x
+#pragma unroll
+                for (int k = 0; k < 4; k++)
+#pragma unroll
+                    for (int i = 0; i < LANES; i++) {
+                        T v = a.c1[fa[k]][0] * (n[k][0][i] - n[k][1][i]);
+                        v = fma_<T>(a.c1[fa[k]][1], n[k][2][i] - n[k][3][i], v);
+                        dd[k][i] = fma_<T>(a.c1[fa[k]][2], n[k][4][i] - n[k][5][i], v);
+                    }
 #pragma unroll
                 for (int i = 0; i < LANES; i++) {
-                    T v = a.c1[axis][0] * (p1[i] - m1[i]);
-                    v = fma_<T>(a.c1[axis][1], p2[i] - m2[i], v);
-                    r[i] = fma_<T>(a.c1[axis][2], p3[i] - m3[i], v);
+                    pbx[s4][tid][i] = dd[0][i];
+                    pby[s4][tid][i] = dd[1][i];
+                    pbz[s4][tid][i] = dd[2][i] - dd[3][i] + a.bext[2];
+                    const double u2 = (double)ux[i] * ux[i] + (double)uy[i] * uy[i] + (double)uz[i] * uz[i];
+                    acc.su += u2;
+                    acc.mu = fmax(acc.mu, u2);
+                    acc.lmin = fmin(acc.lmin, (double)l[i]);
+                    acc.lmax = fmax(acc.lmax, (double)l[i]);
+                    // a non-finite ln rho or A would hide in fmin/fmax: fold it into the sums
+                    const double chk = (double)l[i] + (double)vax[i] + (double)vay[i] + (double)az[i];
+                    if (!isfinite(chk)) acc.su += chk;
                 }
-            };
-            T azy[LANES], ayz[LANES], axz[LANES], azx[LANES], ayx[LANES], axy[LANES];
-            d(AZ, pitch, 1, azy);
-            d(AY, plane, 2, ayz);
-            d(AX, plane, 2, axz);
-            d(AZ, 1, 0, azx);
-            d(AY, 1, 0, ayx);
-            d(AX, pitch, 1, axy);
+            }
 #pragma unroll
             for (int i = 0; i < LANES; i++) {
-                const T bx = azy[i] - ayz[i] + a.bext[0];
-                const T by = axz[i] - azx[i] + a.bext[1];
-                const T bz = ayx[i] - axy[i] + a.bext[2];
-                const double u2 = (double)ux[i] * ux[i] + (double)uy[i] * uy[i] + (double)uz[i] * uz[i];
-                const double b2 = (double)bx * bx + (double)by * by + (double)bz * bz;
-                acc.su += u2;
-                acc.sb += b2;
-                acc.mu = fmax(acc.mu, u2);
-                acc.mb = fmax(acc.mb, b2);
-                acc.lmin = fmin(acc.lmin, (double)l[i]);
-                acc.lmax = fmax(acc.lmax, (double)l[i]);
-                // a non-finite ln rho or A would hide in fmin/fmax: fold it into the sums
-                const double chk = (double)l[i] + (double)ax[i] + (double)ay[i] + (double)az[i];
-                if (!isfinite(chk)) acc.su += chk;
+                hax[s7][tid][i] = vax[i];
+                hay[s7][tid][i] = vay[i];
             }
+            if (p - R >= zs) {                               // plane p - 3 has its 7-plane history: finish B there
+                // slot of plane p - j is (s7 - j) mod 7; plane p - 3 + m  <->  j = 3 - m
+                auto slot7 = [&](int j) { const int t = s7 - j; return t < 0 ? t + 7 : t; };
+                const int q4 = (s4 + 1) & 3;                 // slot of plane p - 3 in the 4-ring
+#pragma unroll
+                for (int i = 0; i < LANES; i++) {
+                    T ayz = a.c1[2][0] * (hay[slot7(2)][tid][i] - hay[slot7(4)][tid][i]);
+                    ayz = fma_<T>(a.c1[2][1], hay[slot7(1)][tid][i] - hay[slot7(5)][tid][i], ayz);
+                    ayz = fma_<T>(a.c1[2][2], vay[i] - hay[slot7(6)][tid][i], ayz);
+                    T axz = a.c1[2][0] * (hax[slot7(2)][tid][i] - hax[slot7(4)][tid][i]);
+                    axz = fma_<T>(a.c1[2][1], hax[slot7(1)][tid][i] - hax[slot7(5)][tid][i], axz);
+                    axz = fma_<T>(a.c1[2][2], vax[i] - hax[slot7(6)][tid][i], axz);
+                    const T bx = pbx[q4][tid][i] - ayz + a.bext[0];
+                    const T by = axz - pby[q4][tid][i] + a.bext[1];
+                    const T bz = pbz[q4][tid][i];
+                    const double b2 = (double)bx * bx + (double)by * by + (double)bz * bz;
+                    acc.sb += b2;
+                    acc.mb = fmax(acc.mb, b2);
+                }
+            }
+            s7 = s7 == 6 ? 0 : s7 + 1;
+            s4 = (s4 + 1) & 3;
         }
     }
     acc = block_reduce(acc);

@@ -59,10 +59,8 @@ def solenoidal_modes(seed, kmax=4):
     return ks, amps
 
 
-def solenoidal_velocity(n, seed, urms=0.1, kmax=4, lengths=(TWO_PI, TWO_PI, TWO_PI)):
-    """Sum over the modes of Re{a exp(i k.x)}, x_a = i_a L_a / n_a, rescaled so that
-    sqrt(mean |u|^2) = urms.  Evaluated with per-axis tables exp(i k_a x_a) contracted axis by
-    axis (a separable sum, no FFT).  Returns (3, nz, ny, nx)."""
+def _solenoidal_components(n, seed, kmax):
+    """Generator of the three unscaled components (nz, ny, nx) of the mode sum, one at a time."""
     nz, ny, nx = _shape(n)
     ks, amps = solenoidal_modes(seed, kmax)
     r = int(kmax)
@@ -75,16 +73,46 @@ def solenoidal_velocity(n, seed, urms=0.1, kmax=4, lengths=(TWO_PI, TWO_PI, TWO_
     ex = np.exp(1j * np.outer(kk, TWO_PI * np.arange(nx) / nx))        # [kx, x]
     ey = np.exp(1j * np.outer(kk, TWO_PI * np.arange(ny) / ny))
     ez = np.exp(1j * np.outer(kk, TWO_PI * np.arange(nz) / nz))
-    u = np.empty((3, nz, ny, nx))
     for c in range(3):
         t1 = np.einsum("abc,cz->abz", coef[c], ez)                     # [kx, ky, z]
         t2 = np.einsum("abz,by->azy", t1, ey)                          # [kx, z, y]
         t2 = np.ascontiguousarray(t2.reshape(nk, nz * ny).T)           # [(z,y), kx]
         # real part of t2 @ ex without forming the complex product
-        u[c] = (t2.real @ ex.real - t2.imag @ ex.imag).reshape(nz, ny, nx)
-    rms = math.sqrt(float((u[0] ** 2 + u[1] ** 2 + u[2] ** 2).mean()))
-    u *= urms / rms
+        yield (t2.real @ ex.real - t2.imag @ ex.imag).reshape(nz, ny, nx)
+
+
+def _sum_sq(a):
+    return float(np.einsum("i,i->", a.ravel(), a.ravel()))
+
+
+def solenoidal_velocity(n, seed, urms=0.1, kmax=4, lengths=(TWO_PI, TWO_PI, TWO_PI)):
+    """Sum over the modes of Re{a exp(i k.x)}, x_a = i_a L_a / n_a, rescaled so that
+    sqrt(mean |u|^2) = urms.  Evaluated with per-axis tables exp(i k_a x_a) contracted axis by
+    axis (a separable sum, no FFT).  Returns (3, nz, ny, nx)."""
+    nz, ny, nx = _shape(n)
+    u = np.empty((3, nz, ny, nx))
+    ssq = 0.0
+    for c, comp in enumerate(_solenoidal_components(n, seed, kmax)):
+        u[c] = comp
+        ssq += _sum_sq(comp)
+    u *= urms / math.sqrt(ssq / (nz * ny * nx))
     return u
+
+
+def solenoidal_state_fields(n, seed, urms=0.1, a_amp=1e-5, kmax=4):
+    """The 7 fields of solenoidal_state(n, seed), one (nz, ny, nx) array at a time and with the
+    same values, holding at most two fields in memory (1024^3: 8.6 GB per field).  The velocity
+    is generated twice: once for its rms, once scaled."""
+    shape = _shape(n)
+    ssq = sum(_sum_sq(comp) for comp in _solenoidal_components(n, seed, kmax))
+    scale = urms / math.sqrt(ssq / (shape[0] * shape[1] * shape[2]))
+    yield np.zeros(shape)
+    for comp in _solenoidal_components(n, seed, kmax):
+        comp *= scale
+        yield comp
+    rng = np.random.default_rng(seed + 1)
+    for _ in range(3):
+        yield rng.standard_normal(shape) * a_amp
 
 
 def solenoidal_state(n, seed, urms=0.1, a_amp=1e-5, kmax=4):
