@@ -24,6 +24,7 @@ class OrcParams(ctypes.Structure):
         ("mixed_mode", ctypes.c_int), ("has_forcing", ctypes.c_int),
         ("fk", ctypes.c_double * 3), ("fphase", ctypes.c_double),
         ("fre", ctypes.c_double * 3), ("fim", ctypes.c_double * 3),
+        ("upwind", ctypes.c_int),
     ]
 
 
@@ -50,6 +51,8 @@ def lib():
         L.orc_der1_field.argtypes = [dp, dp, pp, ctypes.c_int]
         L.orc_der2_field.argtypes = [dp, dp, pp, ctypes.c_int]
         L.orc_dermix_field.argtypes = [dp, dp, pp, ctypes.c_int, ctypes.c_int]
+        L.orc_der6_upwind_field.argtypes = [dp, dp, pp, ctypes.c_int]
+        L.orc_der6_upwind_field.restype = None
         L.orc_max_threads.restype = ctypes.c_int
         L.orc_set_threads.argtypes = [ctypes.c_int]
         for f in (L.orc_rhs, L.orc_substep, L.orc_step, L.orc_diag, L.orc_der1_field, L.orc_der2_field,
@@ -64,7 +67,8 @@ def _ptr(a):
     return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
 
 
-def make_params(shape, lengths, nu=0.0, eta=0.0, cs=1.0, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal"):
+def make_params(shape, lengths, nu=0.0, eta=0.0, cs=1.0, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal",
+                upwind=False):
     nz, ny, nx = shape
     p = OrcParams()
     p.nx, p.ny, p.nz = nx, ny, nz
@@ -72,6 +76,7 @@ def make_params(shape, lengths, nu=0.0, eta=0.0, cs=1.0, forcing=None, bext=(0.0
     p.nu, p.eta, p.cs = nu, eta, cs
     p.bext[:] = bext
     p.mixed_mode = {"bidiagonal": 0, "tensor": 1}[mixed]
+    p.upwind = 1 if upwind else 0
     if forcing is None:
         p.has_forcing = 0
     else:
@@ -84,18 +89,18 @@ def make_params(shape, lengths, nu=0.0, eta=0.0, cs=1.0, forcing=None, bext=(0.0
     return p
 
 
-def rhs(state, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal"):
+def rhs(state, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal", upwind=False):
     state = np.ascontiguousarray(state, dtype=np.float64)
-    p = make_params(state.shape[1:], lengths, nu, eta, cs, forcing, bext, mixed)
+    p = make_params(state.shape[1:], lengths, nu, eta, cs, forcing, bext, mixed, upwind)
     out = np.empty_like(state)
     lib().orc_rhs(_ptr(state), _ptr(out), ctypes.byref(p))
     return out
 
 
-def step(state, dt, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal"):
+def step(state, dt, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal", upwind=False):
     """One full RK3 step; returns a new array."""
     state = np.array(state, dtype=np.float64, order="C", copy=True)
-    p = make_params(state.shape[1:], lengths, nu, eta, cs, forcing, bext, mixed)
+    p = make_params(state.shape[1:], lengths, nu, eta, cs, forcing, bext, mixed, upwind)
     w = np.empty_like(state)
     scratch = np.empty_like(state)
     lib().orc_step(_ptr(state), _ptr(w), _ptr(scratch), float(dt), ctypes.byref(p))
@@ -105,20 +110,21 @@ def step(state, dt, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mi
 class Stepper:
     """Keeps the work arrays so that repeated steps (and the timed baseline) do not reallocate."""
 
-    def __init__(self, state, lengths, nu, eta, cs, bext=(0.0, 0.0, 0.0), mixed="bidiagonal"):
+    def __init__(self, state, lengths, nu, eta, cs, bext=(0.0, 0.0, 0.0), mixed="bidiagonal", upwind=False):
         self.state = np.array(state, dtype=np.float64, order="C", copy=True)
         self.w = np.zeros_like(self.state)
         self.scratch = np.empty_like(self.state)
         self.args = (lengths, nu, eta, cs, bext, mixed)
+        self.upwind = upwind
 
     def step(self, dt, forcing=None):
         lengths, nu, eta, cs, bext, mixed = self.args
-        p = make_params(self.state.shape[1:], lengths, nu, eta, cs, forcing, bext, mixed)
+        p = make_params(self.state.shape[1:], lengths, nu, eta, cs, forcing, bext, mixed, self.upwind)
         lib().orc_step(_ptr(self.state), _ptr(self.w), _ptr(self.scratch), float(dt), ctypes.byref(p))
 
     def substep(self, s, dt, forcing=None):
         lengths, nu, eta, cs, bext, mixed = self.args
-        p = make_params(self.state.shape[1:], lengths, nu, eta, cs, forcing, bext, mixed)
+        p = make_params(self.state.shape[1:], lengths, nu, eta, cs, forcing, bext, mixed, self.upwind)
         lib().orc_substep(_ptr(self.state), _ptr(self.w), _ptr(self.scratch), int(s), float(dt), ctypes.byref(p))
 
     def diagnostics(self):
@@ -148,6 +154,15 @@ def der2_field(f, a, lengths):
     p = make_params(f.shape, lengths)
     out = np.empty_like(f)
     lib().orc_der2_field(_ptr(f), _ptr(out), ctypes.byref(p), a)
+    return out
+
+
+def der6_upwind_field(f, a, lengths):
+    """delta6_a f / (60 h_a) (reading G17)."""
+    f = np.ascontiguousarray(f, dtype=np.float64)
+    p = make_params(f.shape, lengths)
+    out = np.empty_like(f)
+    lib().orc_der6_upwind_field(_ptr(f), _ptr(out), ctypes.byref(p), a)
     return out
 
 

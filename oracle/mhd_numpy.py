@@ -86,6 +86,21 @@ def der2(f, a, h):
     return s / (h[a] * h[a])
 
 
+# 5th-order upwind-biased first derivative on points -3 .. +2 (flow towards +a); the mirror image
+# serves flow towards -a.  Textbook weights (Dobler et al. 2006's upwinding, reading G17), over 60 h.
+UPW5 = (-2.0, 15.0, -60.0, 20.0, 30.0, -3.0)
+
+
+def der1_upwind(f, a, h, vel):
+    """First derivative of f along a taken on the side the flow `vel` comes from."""
+    plus = 0.0      # vel > 0: points -3 .. +2
+    minus = 0.0     # vel < 0: points -2 .. +3 with mirrored, negated weights
+    for w, m in zip(UPW5, (-3, -2, -1, 0, 1, 2)):
+        plus = plus + w * shift(f, a, m)
+        minus = minus - w * shift(f, a, -m)
+    return np.where(vel >= 0.0, plus, minus) / (60.0 * h[a])
+
+
 def dermix(f, a, b, h, mixed="bidiagonal"):
     """D_ab f, a != b.  Default: bidiagonal 12-point stencil (reading G2).
     mixed="tensor" is the alternative reading D_a(D_b f) (36 points), kept as a flag."""
@@ -127,7 +142,7 @@ def forcing_field(shape, h, forcing):
     return [re[i] * c - im[i] * s for i in range(3)]
 
 
-def rhs(state, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal"):
+def rhs(state, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal", upwind=False):
     """Right-hand sides of Eq. 1-3, SURVEY 8(c) steps 2-5."""
     shape = state.shape[1:]
     h = grid_spacing(shape, lengths)
@@ -163,7 +178,13 @@ def rhs(state, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="
 
     # step 4: right-hand sides
     out = np.empty_like(state)
-    out[LNRHO] = -(u[0] * g[0] + u[1] * g[1] + u[2] * g[2]) - divu
+    if upwind:
+        # upwinded continuity equation (reading G17): each u_a d_a ln rho uses the
+        # upwind-biased derivative
+        out[LNRHO] = -(u[0] * der1_upwind(lnrho, 0, h, u[0]) + u[1] * der1_upwind(lnrho, 1, h, u[1])
+                       + u[2] * der1_upwind(lnrho, 2, h, u[2])) - divu
+    else:
+        out[LNRHO] = -(u[0] * g[0] + u[1] * g[1] + u[2] * g[2]) - divu
     rho_inv = np.exp(-lnrho)
     jxb = [jj[1] * B[2] - jj[2] * B[1], jj[2] * B[0] - jj[0] * B[2], jj[0] * B[1] - jj[1] * B[0]]
     uxb = [u[1] * B[2] - u[2] * B[1], u[2] * B[0] - u[0] * B[2], u[0] * B[1] - u[1] * B[0]]
@@ -177,18 +198,19 @@ def rhs(state, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="
     return out
 
 
-def substep(state, w, s, dt, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal"):
+def substep(state, w, s, dt, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal",
+            upwind=False):
     """One 2N-RK3 substep: w <- alpha_s w + dt RHS(f); f <- f + beta_s w."""
-    r = rhs(state, lengths, nu, eta, cs, forcing, bext, mixed)
+    r = rhs(state, lengths, nu, eta, cs, forcing, bext, mixed, upwind)
     w = RK_ALPHA[s] * w + dt * r
     return state + RK_BETA[s] * w, w
 
 
-def step(state, dt, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal"):
+def step(state, dt, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal", upwind=False):
     """One full RK3 step (three substeps, same forcing parameters in all three: reading G8)."""
     w = np.zeros_like(state)
     for s in range(3):
-        state, w = substep(state, w, s, dt, lengths, nu, eta, cs, forcing, bext, mixed)
+        state, w = substep(state, w, s, dt, lengths, nu, eta, cs, forcing, bext, mixed, upwind)
     return state
 
 

@@ -23,6 +23,14 @@
  * (j = grad div A - lap A), G5 (eta times the component-wise Laplacian), G6, G7
  * (Williamson's alpha, beta), G8 (forcing in all three substeps).
  *
+ * Optional (upwind = 1, NEXT-1, reading G17): "In the continuity Equation (1) we have used the
+ * high-order upwinding method of Dobler et al. (2006)" (off in the paper's benchmark,
+ * PAPER.md:533).  The paper prints no formula.  Reading: the advection term -u.grad ln rho keeps
+ * its 6th-order central derivative and gains, per axis a, + |u_a| / (60 h_a) * delta6_a ln rho with
+ * delta6 f = f(-3) - 6 f(-2) + 15 f(-1) - 20 f(0) + 15 f(+1) - 6 f(+2) + f(+3): for u_a > 0 the
+ * sum is exactly the 5th-order upwind-biased stencil (-2, 15, -60, 20, 30, -3, 0) / (60 h) on points
+ * -3 .. +3, mirrored for u_a < 0 (pinned in tests/test_oracle_upwind.py).
+ *
  * Every cell is computed by the same straight-line formula; neighbours are found by
  * wrapping each index modulo the grid size.  No blocking, no fusion across cells, no
  * reordering.  The only parallelism is an OpenMP "parallel for" over z planes.
@@ -48,6 +56,7 @@ typedef struct {
     int mixed_mode;      /* 0 = bidiagonal (default reading), 1 = tensor product D_a(D_b f) */
     int has_forcing;
     double fk[3], fphase, fre[3], fim[3];
+    int upwind;          /* 0 = off (default, all BASELINE configs), 1 = upwinded continuity equation (G17) */
 } orc_params;
 
 static const double C1[3] = {3.0 / 4.0, -3.0 / 20.0, 1.0 / 60.0};
@@ -93,6 +102,20 @@ static double der2(const double* f, const orc_params* p, long x, long y, long z,
     }
     double h = spacing(p, a);
     return s / (h * h);
+}
+
+/* delta6_a f / (60 h_a): the sixth difference that turns the central first derivative into the
+ * 5th-order upwind-biased one (G17) */
+static const double C6_0 = -20.0;
+static const double C6[3] = {15.0, -6.0, 1.0};
+static double der6_upwind(const double* f, const orc_params* p, long x, long y, long z, int a) {
+    double s = C6_0 * at(f, p, x, y, z, 0, 0, 0);
+    for (int m = 1; m <= 3; m++) {
+        long d[3] = {0, 0, 0};
+        d[a] = m;
+        s += C6[m - 1] * (at(f, p, x, y, z, d[0], d[1], d[2]) + at(f, p, x, y, z, -d[0], -d[1], -d[2]));
+    }
+    return s / (60.0 * spacing(p, a));
 }
 
 static double dermix(const double* f, const orc_params* p, long x, long y, long z, int a, int b) {
@@ -170,6 +193,8 @@ void orc_rhs(const double* state, double* rhs, const orc_params* p) {
                 }
                 /* Eq. 1 */
                 rhs[c] = -(uc[0] * g[0] + uc[1] * g[1] + uc[2] * g[2]) - divu;
+                if (p->upwind)
+                    for (int a = 0; a < 3; a++) rhs[c] += fabs(uc[a]) * der6_upwind(lnrho, p, x, y, z, a);
                 /* forcing, Eq. 4 */
                 double f[3] = {0.0, 0.0, 0.0};
                 if (p->has_forcing) {
@@ -258,6 +283,12 @@ void orc_der2_field(const double* f, double* out, const orc_params* p, int a) {
         for (long y = 0; y < p->ny; y++)
             for (long x = 0; x < p->nx; x++)
                 out[(size_t)x + (size_t)p->nx * ((size_t)y + (size_t)p->ny * (size_t)z)] = der2(f, p, x, y, z, a);
+}
+void orc_der6_upwind_field(const double* f, double* out, const orc_params* p, int a) {
+    for (long z = 0; z < p->nz; z++)
+        for (long y = 0; y < p->ny; y++)
+            for (long x = 0; x < p->nx; x++)
+                out[(size_t)x + (size_t)p->nx * ((size_t)y + (size_t)p->ny * (size_t)z)] = der6_upwind(f, p, x, y, z, a);
 }
 void orc_dermix_field(const double* f, double* out, const orc_params* p, int a, int b) {
     for (long z = 0; z < p->nz; z++)
