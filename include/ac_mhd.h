@@ -142,6 +142,12 @@ int ac_make_forcing(const ac_ctx* ctx, uint64_t seed, uint64_t step, double dt, 
  * (defaults 0.4, 0.25).  ac_set_variant: substep kernel variant (0 = default/fastest,
  * others documented in DESIGN.md; AC_EINVAL if unknown). */
 int ac_set_bext(ac_ctx* ctx, const double b[3]);
+/* ac_set_upwind: 1 = the continuity equation uses the high-order upwinding the paper's production
+ * runs used (Dobler et al. 2006; off in its benchmark, and in every
+ * BASELINE config).  Reading G17: -u.grad ln rho keeps the 6th-order central derivative and gains
+ * + sum_a |u_a| / (60 h_a) [f(-3) - 6 f(-2) + 15 f(-1) - 20 f(0) + 15 f(+1) - 6 f(+2) + f(+3)],
+ * which makes each u_a d_a ln rho the 5th-order upwind-biased derivative.  Default 0. */
+int ac_set_upwind(ac_ctx* ctx, int on);
 int ac_set_cfl(ac_ctx* ctx, double c_u, double c_nu);
 int ac_set_variant(ac_ctx* ctx, int variant);
 

@@ -18,6 +18,7 @@ EXPORTS = (
     "ac_workspace_bytes", "ac_init", "ac_load_state", "ac_store_state", "ac_load_field", "ac_store_field", "ac_step",
     "ac_reduce",
     "ac_forcing_from_draws", "ac_forcing_params", "ac_make_forcing", "ac_set_bext", "ac_set_cfl", "ac_set_variant",
+    "ac_set_upwind",
     "ac_launch_count", "ac_free", "ac_strerror", "ac_version",
 )
 
@@ -87,6 +88,8 @@ def load_library():
     L.ac_set_bext.argtypes = [vp, ctypes.POINTER(dbl)]
     L.ac_set_cfl.argtypes = [vp, dbl, dbl]
     L.ac_set_variant.argtypes = [vp, i32]
+    L.ac_set_upwind.argtypes = [vp, i32]
+    L.ac_set_upwind.restype = i32
     L.ac_launch_count.argtypes = [vp]
     L.ac_launch_count.restype = ctypes.c_longlong
     L.ac_free.argtypes = [vp]
@@ -253,6 +256,9 @@ class Context:
 
     def ac_set_variant(self, variant):
         _check(self._lib.ac_set_variant(self._ctx, int(variant)), "ac_set_variant")
+
+    def ac_set_upwind(self, on):
+        _check(self._lib.ac_set_upwind(self._ctx, int(bool(on))), "ac_set_upwind")
 
     def ac_launch_count(self):
         return int(self._lib.ac_launch_count(self._ctx))

@@ -41,6 +41,9 @@ const double W1[3] = {3.0 / 4.0, -3.0 / 20.0, 1.0 / 60.0};
 const double W2_0 = -49.0 / 18.0;
 const double W2[3] = {3.0 / 2.0, -3.0 / 20.0, 1.0 / 90.0};
 const double WM[3] = {3.0 / 8.0, -3.0 / 80.0, 1.0 / 360.0};
+// upwind correction of the continuity equation (G17): delta6 / 60, weights of f(0) and f(+m) + f(-m)
+const double W6_0 = -20.0 / 60.0;
+const double W6[3] = {15.0 / 60.0, -6.0 / 60.0, 1.0 / 60.0};
 const double RK_ALPHA[3] = {0.0, -5.0 / 9.0, -153.0 / 128.0};
 const double RK_BETA[3] = {1.0 / 3.0, 15.0 / 16.0, 8.0 / 15.0};
 
@@ -137,6 +140,7 @@ struct ac_ctx {
     double nu, eta, cs, k_f, helicity;
     double bext[3];
     double c_u, c_nu;
+    int upwind;          // 1 = upwinded continuity equation (G17); default 0
     int variant;         // requested: 0 = scatter-march, 1 = direct
     bool march;          // the kernel actually used (fp32 with odd nz falls back to direct)
     bool packed;         // fp32 cells stored as (z, z + nz/2) pairs
@@ -168,6 +172,8 @@ void fill_coeffs(const ac_ctx* ctx, ac::Coeffs<T>& c) {
             c.c2[a][m] = (T)(W2[m] / (h[a] * h[a]));
         }
         c.c20[a] = (T)(W2_0 / (h[a] * h[a]));
+        c.c60[a] = (T)(W6_0 / h[a]);
+        for (int m = 0; m < 3; m++) c.c6[a][m] = (T)(W6[m] / h[a]);
     }
     const int pa[3] = {0, 0, 1}, pb[3] = {1, 2, 2};
     for (int p = 0; p < 3; p++)
@@ -264,6 +270,14 @@ void fill_march_coef(const ac_ctx* ctx, ac::MarchCoef<E>& c, double dt, int s, c
         }
         c.w20[i] = S::of(fx * c20[0] + fy * c20[1] + fz * c20[2]);
     }
+    for (int m = 0; m < 3; m++) {
+        c.c6x[m] = S::of(W6[m] / h[0]);
+        c.c6y[m] = S::of(W6[m] / h[1]);
+        c.c6z[m] = S::of(W6[m] / h[2]);
+    }
+    c.c60x = S::of(W6_0 / h[0]);
+    c.c60y = S::of(W6_0 / h[1]);
+    c.c60z = S::of(W6_0 / h[2]);
     c.c20all = S::of(c20[0] + c20[1] + c20[2]);
     c.nc20yz = S::of(-(c20[1] + c20[2]));
     c.nc20xz = S::of(-(c20[0] + c20[2]));
@@ -306,8 +320,12 @@ int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
             fill_march_coef<E>(ctx, a.c, dt, s, forcing);
             for (int q = 0; q < AC_NFIELDS; q++) a.out[q] = (E*)ctx->field_ptr(1 - ctx->cur, q);
             dim3 grd((L.nx + ac::M_TX - 1) / ac::M_TX, (L.ny + ac::M_TY - 1) / ac::M_TY, ctx->nchunks);
-            ac::substep_march_kernel<T><<<grd, ac::M_THREADS, ac::M_SMEM_BYTES, ctx->stream>>>(
-                a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
+            if (ctx->upwind)
+                ac::substep_march_kernel<T, true><<<grd, ac::M_THREADS, ac::M_SMEM_BYTES, ctx->stream>>>(
+                    a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
+            else
+                ac::substep_march_kernel<T, false><<<grd, ac::M_THREADS, ac::M_SMEM_BYTES, ctx->stream>>>(
+                    a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
             ctx->launches++;
             // S1: refresh the ghost zones of the buffer just written
             const int nb_rows = 2 * ac::R * L.my + 2 * ac::R * L.nz;
@@ -328,6 +346,7 @@ int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
         a.p.cs2 = (T)(ctx->cs * ctx->cs);
         for (int i = 0; i < 3; i++) a.p.bext[i] = (T)ctx->bext[i];
         a.p.has_forcing = forcing ? 1 : 0;
+        a.p.upwind = ctx->upwind;
         for (int i = 0; i < 3; i++) {
             a.p.fre[i] = forcing ? (T)forcing->re[i] : T(0);
             a.p.fim[i] = forcing ? (T)forcing->im[i] : T(0);
@@ -463,12 +482,14 @@ int configure(ac_ctx* ctx) {
         if (rc == AC_OK) rc = make_state_map(&ctx->map_prev[b], ctx->field_ptr(b, 0), ctx->L, ac::M_TX, ac::M_TY);
         if (rc != AC_OK) return rc;
     }
-    cudaError_t ea = ctx->dtype == AC_F64
-                         ? cudaFuncSetAttribute(ac::substep_march_kernel<double>,
-                                                cudaFuncAttributeMaxDynamicSharedMemorySize, ac::M_SMEM_BYTES)
-                         : cudaFuncSetAttribute(ac::substep_march_kernel<float>,
-                                                cudaFuncAttributeMaxDynamicSharedMemorySize, ac::M_SMEM_BYTES);
-    if (ea != cudaSuccess) return cuda_fail(ea, "cudaFuncSetAttribute(march kernel smem)");
+    const void* kernels[4] = {(const void*)ac::substep_march_kernel<double, false>,
+                              (const void*)ac::substep_march_kernel<double, true>,
+                              (const void*)ac::substep_march_kernel<float, false>,
+                              (const void*)ac::substep_march_kernel<float, true>};
+    for (int k = (ctx->dtype == AC_F64 ? 0 : 2), e = k + 2; k < e; k++) {
+        cudaError_t ea = cudaFuncSetAttribute(kernels[k], cudaFuncAttributeMaxDynamicSharedMemorySize, ac::M_SMEM_BYTES);
+        if (ea != cudaSuccess) return cuda_fail(ea, "cudaFuncSetAttribute(march kernel smem)");
+    }
     // z chunks: every chunk re-reads 6 planes, every wave of CTAs costs (planes + 6) iterations;
     // pick the chunk count that minimises waves x (planes per chunk + 6)
     const int nzp = ctx->L.nz;
@@ -535,6 +556,7 @@ int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double
     ctx->c_u = 0.4;
     ctx->c_nu = 0.25;
     ctx->variant = 0;
+    ctx->upwind = 0;
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->launches = 0;
     ctx->host_result = nullptr;
@@ -716,6 +738,12 @@ int ac_set_cfl(ac_ctx* ctx, double c_u, double c_nu) {
     if (!ctx || !(c_u > 0.0) || !(c_nu > 0.0)) return AC_EINVAL;
     ctx->c_u = c_u;
     ctx->c_nu = c_nu;
+    return AC_OK;
+}
+
+int ac_set_upwind(ac_ctx* ctx, int on) {
+    if (!ctx || (on != 0 && on != 1)) return AC_EINVAL;
+    ctx->upwind = on;
     return AC_OK;
 }
 

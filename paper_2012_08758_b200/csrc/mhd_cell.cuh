@@ -24,6 +24,8 @@ struct Coeffs {
     T c2[3][3];
     T c20[3];
     T cm[3][3];
+    T c6[3][3];   // upwinding (G17): weights (15, -6, 1) / (60 h_a) of f(+m) + f(-m)
+    T c60[3];     //                  centre weight -20 / (60 h_a)
 };
 
 template <typename T>
@@ -35,6 +37,7 @@ struct Physics {
     T fre[3], fim[3];
     int has_forcing;
     int substep;
+    int upwind;   // 1: continuity equation with the 5th-order upwind correction (G17)
 };
 
 template <typename T>
@@ -44,6 +47,8 @@ __device__ __forceinline__ double fma_<double>(double a, double b, double c) { r
 template <>
 __device__ __forceinline__ float fma_<float>(float a, float b, float c) { return fmaf(a, b, c); }
 
+__device__ __forceinline__ double abs_(double x) { return fabs(x); }
+__device__ __forceinline__ float abs_(float x) { return fabsf(x); }
 __device__ __forceinline__ double exp_neg(double x) { return exp(-x); }
 __device__ __forceinline__ float exp_neg(float x) { return expf(-x); }
 
@@ -71,6 +76,16 @@ __device__ __forceinline__ T d2(const F& f, const Coeffs<T>& c, int q, T f0) {
     r = fma_<T>(c.c2[A][0], nb<A>(f, q, 1) + nb<A>(f, q, -1), r);
     r = fma_<T>(c.c2[A][1], nb<A>(f, q, 2) + nb<A>(f, q, -2), r);
     r = fma_<T>(c.c2[A][2], nb<A>(f, q, 3) + nb<A>(f, q, -3), r);
+    return r;
+}
+
+// upwind correction along axis A: delta6_A f / (60 h_A)
+template <typename T, int A, typename F>
+__device__ __forceinline__ T d6(const F& f, const Coeffs<T>& c, int q, T f0) {
+    T r = c.c60[A] * f0;
+    r = fma_<T>(c.c6[A][0], nb<A>(f, q, 1) + nb<A>(f, q, -1), r);
+    r = fma_<T>(c.c6[A][1], nb<A>(f, q, 2) + nb<A>(f, q, -2), r);
+    r = fma_<T>(c.c6[A][2], nb<A>(f, q, 3) + nb<A>(f, q, -3), r);
     return r;
 }
 
@@ -157,6 +172,12 @@ __device__ __forceinline__ void substep_cell(const F& f, const Coeffs<T>& c, con
     // right-hand sides
     T rhs[7];
     rhs[LNRHO] = -(fma_<T>(u[0], g[0], fma_<T>(u[1], g[1], u[2] * g[2]))) - divu;
+    if (p.upwind) {
+        T up = abs_(u[0]) * d6<T, 0>(f, c, LNRHO, lnrho);
+        up = fma_<T>(abs_(u[1]), d6<T, 1>(f, c, LNRHO, lnrho), up);
+        up = fma_<T>(abs_(u[2]), d6<T, 2>(f, c, LNRHO, lnrho), up);
+        rhs[LNRHO] += up;
+    }
 
     const T rho_inv = exp_neg(lnrho);
     const T jxb[3] = {jj[1] * B[2] - jj[2] * B[1], jj[2] * B[0] - jj[0] * B[2], jj[0] * B[1] - jj[1] * B[0]};

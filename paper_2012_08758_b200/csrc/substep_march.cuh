@@ -59,7 +59,7 @@ constexpr int M_NF = 7;
 
 constexpr int M_SLOT_BYTES = M_NF * M_PLANE * 8;        // 18816 (multiple of 128)
 constexpr int M_PSLOT_BYTES = M_NF * M_COLS * 8;        // 7168
-constexpr int M_MBOX_BYTES = 3 * M_COLS * 8;            // 3072 per depth
+constexpr int M_MBOX_BYTES = 4 * M_COLS * 8;            // 4096 per depth: (j x B)/rho and the upwind term
 constexpr int M_OFF_PREV = M_NP * M_SLOT_BYTES;
 constexpr int M_OFF_MBOX = M_OFF_PREV + M_NPP * M_PSLOT_BYTES;
 constexpr int M_OFF_ZTAB = M_OFF_MBOX + M_ND * M_MBOX_BYTES;
@@ -81,6 +81,8 @@ struct MarchCoef {
     E c2x[3], c2y[3], c2z[3], nc2x[3], nc2y[3], nc2z[3];
     E c20all, nc20yz, nc20xz, nc20xy;
     E cmxy[3], cmxz[3], ncmxz[3], cmyz[3], ncmyz[3];
+    // upwind correction of the continuity equation (G17; UPW kernels only): delta6 / (60 h)
+    E c6x[3], c6y[3], c6z[3], c60x, c60y, c60z;
     // physics and time stepping
     E nu, eta, ncs2, bext[3], rk_a, rk_b, fre[3], nfim[3], n23;
 };
@@ -161,6 +163,11 @@ __device__ __forceinline__ void m_diff(const E* p, E (&d)[3]) {
 #pragma unroll
     for (int m = 1; m <= 3; m++) d[m - 1] = vsub(p[m * STRIDE], p[-m * STRIDE]);
 }
+template <typename E, int STRIDE>
+__device__ __forceinline__ void m_sum(const E* p, E (&s)[3]) {
+#pragma unroll
+    for (int m = 1; m <= 3; m++) s[m - 1] = vadd(p[m * STRIDE], p[-m * STRIDE]);
+}
 // in-plane bidiagonal mixed derivative (G2) with weights cm
 template <typename E>
 __device__ __forceinline__ E m_mixxy(const E* p, const E (&cm)[3]) {
@@ -224,7 +231,10 @@ __global__ void __launch_bounds__(M_GHOST_THREADS) ghost_fill_kernel(E* __restri
     }
 }
 
-template <typename T>
+// UPW: continuity equation with the 5th-order upwind correction (G17).  The A role, which has
+// registers to spare, forms  sum_a |u_a| delta6_a ln rho / (60 h_a)  (x, y parts in plane, z part
+// scattered like every other z stencil) and hands it to the U role with (j x B)/rho.
+template <typename T, bool UPW>
 __global__ void __launch_bounds__(M_THREADS, 1)
     substep_march_kernel(const __grid_constant__ MarchArgs<T> a, const __grid_constant__ CUtensorMap map_in,
                          const __grid_constant__ CUtensorMap map_prev) {
@@ -392,7 +402,7 @@ __global__ void __launch_bounds__(M_THREADS, 1)
                 const E* pc = (const E*)(smem + ((k - R) % M_NP) * M_SLOT_BYTES) + cell_off;
                 const E lnrho = pc[0], ux = pc[M_PLANE], uy = pc[2 * M_PLANE], uz = pc[3 * M_PLANE];
                 const E divu = vadd(vadd(Gxx[0], Gyy[0]), Gzz[0]);
-                // (j x B) / rho and grad ln rho from the A role of the same columns
+                // (j x B) / rho (and the upwind term) from the A role of the same columns
                 const int u = k - 2 * R;
                 m_bar_wait(&mfull[pair * M_ND + u % M_ND], (uint32_t)((u / M_ND) & 1));
                 const E* mb = (const E*)(smem + M_OFF_MBOX + (u % M_ND) * M_MBOX_BYTES) + col;
@@ -403,6 +413,7 @@ __global__ void __launch_bounds__(M_THREADS, 1)
                 rl = vfma(uy, g1, rl);
                 rl = vfma(uz, g2, rl);
                 rl = vneg(vadd(rl, divu));
+                if (UPW) rl = vadd(rl, mb[3 * M_COLS]);
                 // forcing Eq. 4: f_i = re_i cos(theta) - im_i sin(theta)
                 E fc = vzero<E>(), fs = vzero<E>();
                 if (a.has_forcing) {
@@ -486,6 +497,11 @@ __global__ void __launch_bounds__(M_THREADS, 1)
         // ======================================= A role ========================================
         E Bx[7], By[7], Px[7], Py[7], Pz[7], Jx[7], Jy[7], Jz[7];   // P_i = lap A_i
         E Bz[4];
+        E u6z[7], u6x[4], u6y[4];                                    // UPW only: delta6 ln rho / (60 h) per axis
+#pragma unroll
+        for (int r = 0; r < 7; r++) u6z[r] = vzero<E>();
+#pragma unroll
+        for (int r = 0; r < 4; r++) u6x[r] = u6y[r] = vzero<E>();
 #pragma unroll
         for (int r = 0; r < 7; r++) Bx[r] = By[r] = Px[r] = Py[r] = Pz[r] = Jx[r] = Jy[r] = Jz[r] = vzero<E>();
 #pragma unroll
@@ -503,6 +519,19 @@ __global__ void __launch_bounds__(M_THREADS, 1)
 
             Bx[6] = By[6] = Px[6] = Py[6] = Pz[6] = Jx[6] = Jy[6] = Jz[6] = vzero<E>();
             E d[3], s[3], e[3], t[3];
+            if (UPW) {
+                // ---- ln rho: sixth differences along x, y (in plane) and z (scattered) ----
+                const E* p = pl;
+                const E f0 = p[0];
+                m_sum<E, 1>(p, s);
+                m_sum<E, M_WX>(p, t);
+                u6x[3] = m_dot3(c.c6x, s, vmul(c.c60x, f0));
+                u6y[3] = m_dot3(c.c6y, t, vmul(c.c60y, f0));
+                u6z[6] = vzero<E>();
+                u6z[3] = vfma(c.c60z, f0, u6z[3]);
+#pragma unroll
+                for (int m = 1; m <= 3; m++) M_SCAT(u6z, m, c.c6z[m - 1], c.c6z[m - 1], f0);
+            }
             // ---- A_x: B_z -= d_y A_x; lap; J_x -= (D_yy + D_zz) A_x; D_xy A_x -> J_y; D_xz A_x -> J_z; B_y += d_z A_x
             {
                 const E* p = pl + 4 * M_PLANE;
@@ -573,6 +602,11 @@ __global__ void __launch_bounds__(M_THREADS, 1)
                 mb[0] = vmul(rho_inv, vsub(vmul(j1, b2), vmul(j2, b1)));
                 mb[M_COLS] = vmul(rho_inv, vsub(vmul(j2, b0), vmul(j0, b2)));
                 mb[2 * M_COLS] = vmul(rho_inv, vsub(vmul(j0, b1), vmul(j1, b0)));
+                if (UPW) {
+                    E up = vmul(vabs(pc[M_PLANE]), u6x[0]);
+                    up = vfma(vabs(pc[2 * M_PLANE]), u6y[0], up);
+                    mb[3 * M_COLS] = vfma(vabs(pc[3 * M_PLANE]), u6z[0], up);
+                }
                 __syncwarp();
                 if (lane == 0) m_bar_arrive(&mfull[pair * M_ND + u % M_ND]);
                 const E ux = pc[M_PLANE], uy = pc[2 * M_PLANE], uz = pc[3 * M_PLANE];
@@ -607,6 +641,12 @@ __global__ void __launch_bounds__(M_THREADS, 1)
             }
 #pragma unroll
             for (int r = 0; r < 3; r++) Bz[r] = Bz[r + 1];
+            if (UPW) {
+#pragma unroll
+                for (int r = 0; r < 6; r++) u6z[r] = u6z[r + 1];
+#pragma unroll
+                for (int r = 0; r < 3; r++) { u6x[r] = u6x[r + 1]; u6y[r] = u6y[r + 1]; }
+            }
         }
     }
 }

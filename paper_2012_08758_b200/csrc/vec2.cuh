@@ -60,6 +60,7 @@ __device__ __forceinline__ double vsub(double a, double b) { return a - b; }
 __device__ __forceinline__ double vmul(double a, double b) { return a * b; }
 __device__ __forceinline__ double vfma(double a, double b, double c) { return fma(a, b, c); }
 __device__ __forceinline__ double vneg(double a) { return -a; }
+__device__ __forceinline__ double vabs(double a) { return fabs(a); }
 __device__ __forceinline__ double vexpneg(double a) { return exp(-a); }
 __device__ __forceinline__ double vswap(double a) { return a; }
 __device__ __forceinline__ double vmake(double lo, double) { return lo; }
@@ -96,6 +97,11 @@ __device__ __forceinline__ void vunpack(f2 a, float& lo, float& hi) {
 __device__ __forceinline__ f2 vneg(f2 a) {
     f2 r;
     r.v = a.v ^ 0x8000000080000000ull;
+    return r;
+}
+__device__ __forceinline__ f2 vabs(f2 a) {
+    f2 r;
+    r.v = a.v & 0x7fffffff7fffffffull;
     return r;
 }
 __device__ __forceinline__ f2 vexpneg(f2 a) {

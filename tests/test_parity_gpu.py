@@ -295,3 +295,40 @@ def test_p16_periodic_replication_1024cubed_fp64():
     ctx.ac_free()
     print("P16 worst group-scaled error", worst)
     assert worst <= 1e-12
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("dtype", [binding.AC_F64, binding.AC_F32])
+def test_next1_upwinded_continuity_equation(variant, dtype):
+    """NEXT-1 (reading G17): ac_set_upwind(1) against the oracle's upwind flag, on a state
+    whose ln rho is rough enough for the sixth differences to matter, non-cubic grid, 1 and 5 steps."""
+    shape = (40, 24, 36)
+    lengths = (2 * math.pi, 1.5 * math.pi, 2.5 * math.pi)
+    npdt = np.float64 if dtype == binding.AC_F64 else np.float32
+    state = inputs.smooth_strong_state(shape, 21)
+    state[0] += 0.02 * (inputs.uniform_state(shape, 22)[0] - 0.5)
+    state[1:4] *= 3.0                                           # |u| up to ~1: the correction is O(1) of the advection term
+    state = state.astype(npdt)
+    nu, dt = 5e-3, 2e-3
+    ctx = make_ctx(shape, dtype=dtype, lengths=lengths, nu=nu, eta=nu, k_f=3, helicity=0.5, variant=variant)
+    ctx.ac_set_upwind(True)
+    ctx.ac_load_state(state)
+    st = mhd_c.Stepper(state.astype(np.float64), lengths, nu, nu, 1.0, upwind=True)
+    plain = mhd_c.Stepper(state.astype(np.float64), lengths, nu, nu, 1.0, upwind=False)
+    nsteps = 5 if dtype == binding.AC_F64 else 1
+    for s in range(nsteps):
+        f = helpers.oracle_forcing(5, s, 3, 0.5, dt, 0.02, 1.0, lengths)
+        ctx.ac_step(dt, ctx.ac_make_forcing(5, s, dt, 0.02))
+        st.step(dt, f)
+        plain.step(dt, f)
+        if s == 0:
+            err1 = helpers.max_group_error(ctx.ac_store_state(), st.state)
+    errn = helpers.max_group_error(ctx.ac_store_state(), st.state)
+    ctx.ac_free()
+    differs = helpers.max_group_error(plain.state, st.state)
+    print("upwind parity", variant, npdt.__name__, err1, errn, "upwind vs central", differs)
+    assert differs > 1e-6                                       # the flag does something
+    if dtype == binding.AC_F64:
+        assert err1 <= 1e-12 and errn <= 1e-11
+    else:
+        assert err1 <= 1e-5
