@@ -332,3 +332,50 @@ def test_next1_upwinded_continuity_equation(variant, dtype):
         assert err1 <= 1e-12 and errn <= 1e-11
     else:
         assert err1 <= 1e-5
+
+
+@pytest.mark.parametrize("shape", [(8, 8, 8), (12, 20, 36), (9, 11, 44), (34, 17, 52)])
+def test_fp32_ragged_grids_packed_and_unpacked(shape):
+    """fp32 on grids that are not multiples of the 16 x 8 tile; odd nz cannot be stored as (z, z + nz/2)
+    pairs and runs the direct kernel, even nz runs the packed march kernel (nz/2 as small as 4 planes)."""
+    state = inputs.gaussian_state(shape, 4, u_amp=1e-2, a_amp=1e-3)
+    state[0] = 0.1 * inputs.uniform_state(shape, 5)[0]
+    state32 = state.astype(np.float32)
+    dt = 1e-3
+    ctx = make_ctx(shape, dtype=binding.AC_F32, nu=1e-2, eta=1e-2, helicity=1.0)
+    ctx.ac_load_state(state32)
+    ctx.ac_step(dt, ctx.ac_make_forcing(3, 0, dt, 0.02))
+    got = ctx.ac_store_state()
+    d = ctx.ac_reduce()
+    ctx.ac_free()
+    want = helpers.oracle_run(state32.astype(np.float64), 1, dt, TWO_PI3, 1e-2, 1e-2, 1.0,
+                              lambda s: helpers.oracle_forcing(3, s, 3, 1.0, dt, 0.02, 1.0))[0]
+    assert helpers.max_group_error(got, want) <= 1e-5, shape
+    dw = mhd_c.diagnostics(want, TWO_PI3)
+    for key in ("urms", "umax", "brms", "bmax"):
+        assert abs(d[key] - dw[key]) <= 2e-5 * dw[key], (shape, key)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("shape", [(8, 8, 8), (40, 9, 72), (33, 64, 28), (96, 40, 24)])
+def test_s9_reductions_match_the_oracle_on_ragged_grids(variant, shape):
+    """S9: rms/max of |u| and |B| (B_ext included), min/max of ln rho and the CFL dt on grids that are
+    not multiples of the reduction kernel's 32 x 8 x 32 work items; run twice: deterministic bits."""
+    lengths = (2 * math.pi, 1.3 * math.pi, 2.9 * math.pi)
+    state = inputs.gaussian_state(shape, 11, u_amp=0.2, a_amp=0.05)
+    state[0] = 0.3 * (inputs.uniform_state(shape, 12)[0] - 0.5)
+    bext = (0.01, -0.02, 0.03)
+    ctx = make_ctx(shape, lengths=lengths, nu=3e-3, eta=1e-3, variant=variant)
+    ctx.ac_set_bext(bext)
+    ctx.ac_load_state(state)
+    d1, d2 = ctx.ac_reduce(), ctx.ac_reduce()
+    ctx.ac_free()
+    assert d1 == d2
+    dw = mhd_c.diagnostics(state, lengths, bext)
+    for key in ("urms", "umax", "brms", "bmax"):
+        assert abs(d1[key] - dw[key]) <= 1e-12 * dw[key], (shape, key)
+    assert d1["lnrho_min"] == dw["lnrho_min"] and d1["lnrho_max"] == dw["lnrho_max"]
+    nz, ny, nx = shape
+    h = min(lengths[0] / nx, lengths[1] / ny, lengths[2] / nz)
+    dt = min(0.4 * h / (dw["umax"] + 1.0), 0.25 * h * h / 3e-3)
+    assert abs(d1["dt_cfl"] - dt) <= 1e-12 * dt
