@@ -29,10 +29,14 @@
 // the loop's code size; profiles/r01b_march.md).
 //
 // Synchronisation: no block-wide barrier in the loop.  full[slot] (TMA transaction bytes) and
-// done[iteration] (one arrival per warp) mbarriers; the first lane of the A role (which runs ahead of
-// the U role) refills ring slots 3 planes ahead once every warp has finished the iteration that
-// last read them.  The A role hands
-// (j x B) to the U role of the same columns through a mailbox with one mbarrier per warp pair.
+// done[iteration] (one arrival per worker warp) mbarriers.  Three warpgroups of 128 threads: U, A and a
+// producer whose single working lane refills ring slots 3 planes ahead once every worker warp has
+// finished the iteration that last read them.  The CTA is launched with 168 registers per thread;
+// setmaxnreg moves the producer's share to the workers (232 each, 40 for the producer).  Giving the
+// producer duty to a lane of a worker warp made that warp run every plane twice (the lane diverges
+// through the wait loop and does not reconverge), the slowest scheduler then held up the whole CTA.
+// The A role hands (j x B)/rho (and the upwind term) to the U role of the same columns through a
+// mailbox with one mbarrier per warp pair.
 //
 // Element type E (vec2.cuh): double, or f2 = two fp32 cells (z, z + nz/2) per element.
 #pragma once
@@ -45,7 +49,10 @@
 
 namespace ac {
 
-constexpr int M_TX = 16, M_TY = 8, M_COLS = M_TX * M_TY, M_THREADS = 2 * M_COLS;
+constexpr int M_TX = 16, M_TY = 8, M_COLS = M_TX * M_TY;
+constexpr int M_WORKERS = 2 * M_COLS;          // U and A roles
+constexpr int M_THREADS = M_WORKERS + 128;    // + the producer warpgroup (one working lane) that feeds the ring
+constexpr int M_REGS_WORKER = 232, M_REGS_PRODUCER = 40;   // setmaxnreg: 128 x (232 + 232 + 40) = 384 x 168, the registers the CTA is launched with
 constexpr int M_HX = 4;                  // x halo of the tile in shared memory (>= R; 32 bytes keeps TMA boxes aligned)
 constexpr int M_WX = M_TX + 2 * M_HX;    // 24
 constexpr int M_WY = M_TY + 2 * R;       // 14
@@ -111,19 +118,37 @@ __device__ __forceinline__ void m_bar_expect_tx(uint64_t* bar, uint32_t bytes) {
 __device__ __forceinline__ void m_bar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(m_smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void m_bar_wait(uint64_t* bar, uint32_t parity) {
+__device__ __forceinline__ bool m_bar_try(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "MWAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
-        "@p bra MDONE_%=;\n"
-        "bra MWAIT_%=;\n"
-        "MDONE_%=:\n"
-        "}\n" ::"r"(m_smem_u32(bar)),
-        "r"(parity), "r"(0x4000u)      // suspend-time hint (ns): fewer polls of a role that runs ahead
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(m_smem_u32(bar)), "r"(parity)
         : "memory");
+    return ok != 0;
 }
+// try_wait suspends the warp for a hardware-limited time by itself; SLEEP_NS > 0 adds a nanosleep between polls
+template <int SLEEP_NS>
+__device__ __forceinline__ void m_bar_wait(uint64_t* bar, uint32_t parity) {
+    while (!m_bar_try(bar, parity)) {
+        if (SLEEP_NS > 0) __nanosleep(SLEEP_NS);
+    }
+}
+// Measured at 512^3 on B200 (16 combinations of 0 / 20 ns at the four wait sites): the fp64 kernel is fastest
+// (21.7 ms per step against 22.7 without any sleep and 28.5 with the U role sleeping alone) when the U role
+// sleeps at the mailbox and the A role at the ring; the packed fp32 kernel is fastest without any sleep
+// (10.85 against 11.3-11.9 ms).  Swapping which role gets the higher warp ids made no difference.
+template <typename T>
+struct MarchWait {
+    static constexpr int MAILBOX_NS = ElemOf<T>::LANES == 1 ? 20 : 0;   // U role waiting for (j x B)/rho
+    static constexpr int RING_A_NS = ElemOf<T>::LANES == 1 ? 20 : 0;    // A role waiting for its next plane
+    static constexpr int RING_U_NS = 0;
+    static constexpr int PRODUCER_NS = 20;
+};
 __device__ __forceinline__ void m_tma_load_4d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2,
                                               int c3) {
     asm volatile(
@@ -250,7 +275,7 @@ __global__ void __launch_bounds__(M_THREADS, 1)
     const Layout& L = a.L;
     const MarchCoef<E>& c = a.c;
     const int tid = threadIdx.x;
-    const int role = tid >> 7;              // 0 = U (ln rho, u), 1 = A
+    const int role = tid >> 7;              // 0 = U (ln rho, u), 1 = A, 2 = producer (one working lane)
     const int col = tid & (M_COLS - 1);
     const int tx = col & (M_TX - 1), ty = col >> 4;
     const int lane = tid & 31;
@@ -266,7 +291,7 @@ __global__ void __launch_bounds__(M_THREADS, 1)
     if (tid == 0) {
         for (int s = 0; s < M_NP; s++) {
             m_bar_init(&full[s], 1);
-            m_bar_init(&done[s], M_THREADS / 32);
+            m_bar_init(&done[s], M_WORKERS / 32);
         }
         for (int s = 0; s < 4 * M_ND; s++) m_bar_init(&mfull[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -293,8 +318,25 @@ __global__ void __launch_bounds__(M_THREADS, 1)
             m_tma_load_4d(smem + M_OFF_PREV + (k % M_NPP) * M_PSLOT_BYTES, &map_prev, &full[slot], x0 + L.gx, y0 + R,
                           zs + k - R, 0);
     };
-    if (tid == M_COLS)
-        for (int k = 0; k < M_LEAD && k < niter; k++) issue(k);
+    // the kernel is launched with 168 registers per thread (384 threads); the producer warpgroup hands its
+    // share to the two worker warpgroups
+    if (role == 2) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(M_REGS_PRODUCER));
+    } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(M_REGS_WORKER));
+    }
+    if (role == 2) {
+        // ===================================== producer warp =====================================
+        // plane k + LEAD reuses the ring slot that every worker warp has released after iteration k - 2
+        if (tid == M_WORKERS) {
+            for (int k = 0; k < M_LEAD && k < niter; k++) issue(k);
+            for (int k = 0; k + M_LEAD < niter; k++) {
+                if (k >= 2) m_bar_wait<MarchWait<T>::PRODUCER_NS>(&done[(k - 2) % M_NP], (uint32_t)(((k - 2) / M_NP) & 1));
+                issue(k + M_LEAD);
+            }
+        }
+        return;
+    }
 
     const int cell_off = (ty + R) * M_WX + tx + M_HX;
 
@@ -322,7 +364,7 @@ __global__ void __launch_bounds__(M_THREADS, 1)
         for (int r = 0; r < 4; r++) Gxx[r] = Gxy[r] = Gyx[r] = Gyy[r] = Gzx[r] = Gzy[r] = vzero<E>();
 
         for (int k = 0; k < niter; k++) {
-            m_bar_wait(&full[k % M_NP], (uint32_t)((k / M_NP) & 1));
+            m_bar_wait<MarchWait<T>::RING_U_NS>(&full[k % M_NP], (uint32_t)((k / M_NP) & 1));
             const E* pl = (const E*)(smem + (k % M_NP) * M_SLOT_BYTES) + cell_off;
 
             Gxz[6] = Gyz[6] = Gzz[6] = Lx[6] = Ly[6] = Lz[6] = vzero<E>();
@@ -404,7 +446,7 @@ __global__ void __launch_bounds__(M_THREADS, 1)
                 const E divu = vadd(vadd(Gxx[0], Gyy[0]), Gzz[0]);
                 // (j x B) / rho (and the upwind term) from the A role of the same columns
                 const int u = k - 2 * R;
-                m_bar_wait(&mfull[pair * M_ND + u % M_ND], (uint32_t)((u / M_ND) & 1));
+                m_bar_wait<MarchWait<T>::MAILBOX_NS>(&mfull[pair * M_ND + u % M_ND], (uint32_t)((u / M_ND) & 1));
                 const E* mb = (const E*)(smem + M_OFF_MBOX + (u % M_ND) * M_MBOX_BYTES) + col;
                 const E jxb0 = mb[0], jxb1 = mb[M_COLS], jxb2 = mb[2 * M_COLS];
                 const E g0 = gx[0], g1 = gy[0], g2 = gz[0];
@@ -508,13 +550,7 @@ __global__ void __launch_bounds__(M_THREADS, 1)
         for (int r = 0; r < 4; r++) Bz[r] = vzero<E>();
 
         for (int k = 0; k < niter; k++) {
-            // this role runs ahead of the U role, so its first lane also feeds the ring: plane
-            // k + LEAD reuses the slot that every warp has released after iteration k - 2
-            if (tid == M_COLS && k + M_LEAD < niter) {
-                if (k >= 2) m_bar_wait(&done[(k - 2) % M_NP], (uint32_t)(((k - 2) / M_NP) & 1));
-                issue(k + M_LEAD);
-            }
-            m_bar_wait(&full[k % M_NP], (uint32_t)((k / M_NP) & 1));
+            m_bar_wait<MarchWait<T>::RING_A_NS>(&full[k % M_NP], (uint32_t)((k / M_NP) & 1));
             const E* pl = (const E*)(smem + (k % M_NP) * M_SLOT_BYTES) + cell_off;
 
             Bx[6] = By[6] = Px[6] = Py[6] = Pz[6] = Jx[6] = Jy[6] = Jz[6] = vzero<E>();
