@@ -141,13 +141,15 @@ __device__ __forceinline__ void m_bar_wait(uint64_t* bar, uint32_t parity) {
 // Measured at 512^3 on B200 (16 combinations of 0 / 20 ns at the four wait sites): the fp64 kernel is fastest
 // (21.7 ms per step against 22.7 without any sleep and 28.5 with the U role sleeping alone) when the U role
 // sleeps at the mailbox and the A role at the ring; the packed fp32 kernel is fastest without any sleep
-// (10.85 against 11.3-11.9 ms).  Swapping which role gets the higher warp ids made no difference.
+// (10.85 against 11.3-11.9 ms).  Swapping which role gets the higher warp ids made no difference.  Over 40
+// steps both kernels run into the 1000 W power cap (SM clock 1725 MHz fp64 / 1845 MHz fp32: 22.5 / 11.4 ms);
+// the ranking of the policies stays the same there and longer sleeps change nothing.
 template <typename T>
 struct MarchWait {
     static constexpr int MAILBOX_NS = ElemOf<T>::LANES == 1 ? 20 : 0;   // U role waiting for (j x B)/rho
     static constexpr int RING_A_NS = ElemOf<T>::LANES == 1 ? 20 : 0;    // A role waiting for its next plane
     static constexpr int RING_U_NS = 0;
-    static constexpr int PRODUCER_NS = 20;
+    static constexpr int PRODUCER_NS = 200;   // once per plane (~1 us); 20 ns polled 54 times per plane for nothing
 };
 __device__ __forceinline__ void m_tma_load_4d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2,
                                               int c3) {
