@@ -122,6 +122,21 @@ def time_oracle(n_sample, cfg, steps, warmup=0):
     return n_sample ** 3 / float(np.mean(times)), float(np.mean(times)), mhd_c.max_threads()
 
 
+def max_over_ranks(ms, dist, device):
+    """The slowest rank's time (the contract's max-over-ranks), identical on every rank."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(n, world, ms_per_step):
+    """Replicas only: every rank advances its own n^3 box, value = all ranks' cell updates / slowest rank's time."""
+    return world * n ** 3 / (ms_per_step * 1e-3)
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -206,13 +221,10 @@ def run_ours(args):
         launches = ctx.ac_launch_count() - l0
         total_ms = ev[0].elapsed_time(ev[-1])
         per = np.array([ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)])
-        if dist is not None:
-            t = torch.tensor([total_ms], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            total_ms = float(t.item())
+        total_ms = max_over_ranks(total_ms, dist, "cuda")
         diag = ctx.ac_reduce()
         ms_per_step = total_ms / args.steps
-        value = world * n ** 3 / (ms_per_step * 1e-3)
+        value = whole_job_value(n, world, ms_per_step)
         peak, peak_src = measured_peak()
         alg_bytes_launch = WORDS_PER_CELL_STEP / 3.0 * es * n ** 3         # average over the 3 substep launches
         launch_ms = ms_per_step / 3.0
@@ -247,12 +259,9 @@ def run_ours(args):
             e1.record(ctx.stream)
             torch.cuda.synchronize()
             e2e_ms = e0.elapsed_time(e1) / k_e2e
-            if dist is not None:
-                t = torch.tensor([e2e_ms], device="cuda")
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                e2e_ms = float(t.item())
+            e2e_ms = max_over_ranks(e2e_ms, dist, "cuda")
             nbytes = 7 * n ** 3 * es
-            res["e2e"] = {"value": world * n ** 3 / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+            res["e2e"] = {"value": whole_job_value(n, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": nbytes,
                           "d2h_bytes_per_step": nbytes, "ms_per_step": e2e_ms, "steps": k_e2e,
                           "what": "ac_load_state(pinned host) + ac_step + ac_store_state(pinned host) per step"}
             del out
