@@ -148,6 +148,11 @@ int ac_set_bext(ac_ctx* ctx, const double b[3]);
  * + sum_a |u_a| / (60 h_a) [f(-3) - 6 f(-2) + 15 f(-1) - 20 f(0) + 15 f(+1) - 6 f(+2) + f(+3)],
  * which makes each u_a d_a ln rho the 5th-order upwind-biased derivative.  Default 0. */
 int ac_set_upwind(ac_ctx* ctx, int on);
+/* ac_set_mixed: reading of the mixed-derivative scheme, which the paper does not print (G2).  0 (default, all
+ * reported parity and every BASELINE config) = bidiagonal 12-point stencil; 1 = tensor product D_a(D_b f), 36
+ * points, also radius 3 and 6th order.  Mode 1 runs the direct kernel whatever the variant.  Like ac_set_variant
+ * it must be called before ac_load_state (a loaded state is dropped: AC_ESTATE until the next load). */
+int ac_set_mixed(ac_ctx* ctx, int mode);
 int ac_set_cfl(ac_ctx* ctx, double c_u, double c_nu);
 int ac_set_variant(ac_ctx* ctx, int variant);
 

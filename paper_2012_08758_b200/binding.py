@@ -18,7 +18,7 @@ EXPORTS = (
     "ac_workspace_bytes", "ac_init", "ac_load_state", "ac_store_state", "ac_load_field", "ac_store_field", "ac_step",
     "ac_reduce",
     "ac_forcing_from_draws", "ac_forcing_params", "ac_make_forcing", "ac_set_bext", "ac_set_cfl", "ac_set_variant",
-    "ac_set_upwind",
+    "ac_set_upwind", "ac_set_mixed",
     "ac_launch_count", "ac_free", "ac_strerror", "ac_version",
 )
 
@@ -90,6 +90,8 @@ def load_library():
     L.ac_set_variant.argtypes = [vp, i32]
     L.ac_set_upwind.argtypes = [vp, i32]
     L.ac_set_upwind.restype = i32
+    L.ac_set_mixed.argtypes = [vp, i32]
+    L.ac_set_mixed.restype = i32
     L.ac_launch_count.argtypes = [vp]
     L.ac_launch_count.restype = ctypes.c_longlong
     L.ac_free.argtypes = [vp]
@@ -259,6 +261,11 @@ class Context:
 
     def ac_set_upwind(self, on):
         _check(self._lib.ac_set_upwind(self._ctx, int(bool(on))), "ac_set_upwind")
+
+    def ac_set_mixed(self, mode):
+        """0 / "bidiagonal" (default) or 1 / "tensor"."""
+        mode = {"bidiagonal": 0, "tensor": 1}.get(mode, mode)
+        _check(self._lib.ac_set_mixed(self._ctx, int(mode)), "ac_set_mixed")
 
     def ac_launch_count(self):
         return int(self._lib.ac_launch_count(self._ctx))

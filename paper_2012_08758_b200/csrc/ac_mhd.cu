@@ -141,6 +141,7 @@ struct ac_ctx {
     double bext[3];
     double c_u, c_nu;
     int upwind;          // 1 = upwinded continuity equation (G17); default 0
+    int mixed;           // 0 = bidiagonal mixed stencil (G2, default), 1 = tensor product (direct kernel only)
     int variant;         // requested: 0 = scatter-march, 1 = direct
     bool march;          // the kernel actually used (fp32 with odd nz falls back to direct)
     bool packed;         // fp32 cells stored as (z, z + nz/2) pairs
@@ -347,6 +348,7 @@ int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
         for (int i = 0; i < 3; i++) a.p.bext[i] = (T)ctx->bext[i];
         a.p.has_forcing = forcing ? 1 : 0;
         a.p.upwind = ctx->upwind;
+        a.p.mixed_tensor = ctx->mixed;
         for (int i = 0; i < 3; i++) {
             a.p.fre[i] = forcing ? (T)forcing->re[i] : T(0);
             a.p.fim[i] = forcing ? (T)forcing->im[i] : T(0);
@@ -469,7 +471,7 @@ namespace {
 // choose the kernel and the device layout for the context's variant; builds the TMA maps
 int configure(ac_ctx* ctx) {
     const ac_grid* g = &ctx->grid;
-    ctx->march = ctx->variant == 0 && (ctx->dtype == AC_F64 || can_pack(g));
+    ctx->march = ctx->variant == 0 && ctx->mixed == 0 && (ctx->dtype == AC_F64 || can_pack(g));
     ctx->packed = ctx->march && ctx->dtype == AC_F32;
     ctx->L = layout_for(g, ctx->dtype, ctx->packed);
     ctx->cv = carve(ctx->L, store_elem_size(ctx->dtype, ctx->packed), elem_size(ctx->dtype), g->nz);
@@ -557,6 +559,7 @@ int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double
     ctx->c_nu = 0.25;
     ctx->variant = 0;
     ctx->upwind = 0;
+    ctx->mixed = 0;
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->launches = 0;
     ctx->host_result = nullptr;
@@ -745,6 +748,15 @@ int ac_set_upwind(ac_ctx* ctx, int on) {
     if (!ctx || (on != 0 && on != 1)) return AC_EINVAL;
     ctx->upwind = on;
     return AC_OK;
+}
+
+int ac_set_mixed(ac_ctx* ctx, int mode) {
+    if (!ctx || (mode != 0 && mode != 1)) return AC_EINVAL;
+    if (mode == ctx->mixed) return AC_OK;
+    // the tensor-product reading exists in the direct kernel only, whose fp32 device layout differs
+    cudaStreamSynchronize(ctx->stream);
+    ctx->mixed = mode;
+    return configure(ctx);
 }
 
 int ac_set_variant(ac_ctx* ctx, int variant) {

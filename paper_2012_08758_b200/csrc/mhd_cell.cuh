@@ -38,6 +38,7 @@ struct Physics {
     int has_forcing;
     int substep;
     int upwind;   // 1: continuity equation with the 5th-order upwind correction (G17)
+    int mixed_tensor;   // 1: mixed derivatives as D_a(D_b f) (36 points) instead of the bidiagonal stencil (G2, NEXT-4)
 };
 
 template <typename T>
@@ -97,11 +98,26 @@ __device__ __forceinline__ auto corner(const F& f, int q, int sa, int sb) {
     return f(q, d[0], d[1], d[2]);
 }
 
-// mixed derivative in the plane of axes A < B, bidiagonal 12-point stencil (G2)
+// mixed derivative in the plane of axes A < B: bidiagonal 12-point stencil (G2, the default reading), or, with
+// tensor = true, the alternative reading D_A(D_B f) = first-derivative stencil along A of first derivatives
+// along B (36 points, same radius; NEXT-4)
 template <typename T, int A, int B, typename F>
-__device__ __forceinline__ T dmix(const F& f, const Coeffs<T>& c, int q) {
+__device__ __forceinline__ T dmix(const F& f, const Coeffs<T>& c, int q, bool tensor) {
     constexpr int P = (A == 0 && B == 1) ? 0 : ((A == 0 && B == 2) ? 1 : 2);
     T r = T(0);
+    if (tensor) {
+#pragma unroll
+        for (int m = 1; m <= 3; m++) {
+            T dp = T(0), dm = T(0);     // D_B f at +m e_A and at -m e_A
+#pragma unroll
+            for (int n = 1; n <= 3; n++) {
+                dp = fma_<T>(c.c1[B][n - 1], corner<A, B>(f, q, m, n) - corner<A, B>(f, q, m, -n), dp);
+                dm = fma_<T>(c.c1[B][n - 1], corner<A, B>(f, q, -m, n) - corner<A, B>(f, q, -m, -n), dm);
+            }
+            r = fma_<T>(c.c1[A][m - 1], dp - dm, r);
+        }
+        return r;
+    }
 #pragma unroll
     for (int m = 1; m <= 3; m++) {
         T s = (corner<A, B>(f, q, m, m) + corner<A, B>(f, q, -m, -m)) -
@@ -143,11 +159,12 @@ __device__ __forceinline__ void substep_cell(const F& f, const Coeffs<T>& c, con
         u2[i][1] = d2<T, 1>(f, c, UX + i, u[i]);
         u2[i][2] = d2<T, 2>(f, c, UX + i, u[i]);
     }
+    const bool mt = p.mixed_tensor != 0;
     // grad div u: diagonal second derivative + two mixed derivatives (G3)
     T gdu[3];
-    gdu[0] = u2[0][0] + dmix<T, 0, 1>(f, c, UY) + dmix<T, 0, 2>(f, c, UZ);
-    gdu[1] = u2[1][1] + dmix<T, 0, 1>(f, c, UX) + dmix<T, 1, 2>(f, c, UZ);
-    gdu[2] = u2[2][2] + dmix<T, 0, 2>(f, c, UX) + dmix<T, 1, 2>(f, c, UY);
+    gdu[0] = u2[0][0] + dmix<T, 0, 1>(f, c, UY, mt) + dmix<T, 0, 2>(f, c, UZ, mt);
+    gdu[1] = u2[1][1] + dmix<T, 0, 1>(f, c, UX, mt) + dmix<T, 1, 2>(f, c, UZ, mt);
+    gdu[2] = u2[2][2] + dmix<T, 0, 2>(f, c, UX, mt) + dmix<T, 1, 2>(f, c, UY, mt);
 
     // magnetic field, Laplacian of A, current density
     T B[3];
@@ -165,9 +182,9 @@ __device__ __forceinline__ void substep_cell(const F& f, const Coeffs<T>& c, con
 #pragma unroll
     for (int i = 0; i < 3; i++) lapA[i] = a2[i][0] + a2[i][1] + a2[i][2];
     // j_i = d_ii A_i + sum_{j != i} d_ij A_j - lap A_i = mixed terms - the other two second derivatives
-    jj[0] = dmix<T, 0, 1>(f, c, AY) + dmix<T, 0, 2>(f, c, AZ) - (a2[0][1] + a2[0][2]);
-    jj[1] = dmix<T, 0, 1>(f, c, AX) + dmix<T, 1, 2>(f, c, AZ) - (a2[1][0] + a2[1][2]);
-    jj[2] = dmix<T, 0, 2>(f, c, AX) + dmix<T, 1, 2>(f, c, AY) - (a2[2][0] + a2[2][1]);
+    jj[0] = dmix<T, 0, 1>(f, c, AY, mt) + dmix<T, 0, 2>(f, c, AZ, mt) - (a2[0][1] + a2[0][2]);
+    jj[1] = dmix<T, 0, 1>(f, c, AX, mt) + dmix<T, 1, 2>(f, c, AZ, mt) - (a2[1][0] + a2[1][2]);
+    jj[2] = dmix<T, 0, 2>(f, c, AX, mt) + dmix<T, 1, 2>(f, c, AY, mt) - (a2[2][0] + a2[2][1]);
 
     // right-hand sides
     T rhs[7];

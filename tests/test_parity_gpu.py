@@ -379,3 +379,29 @@ def test_s9_reductions_match_the_oracle_on_ragged_grids(variant, shape):
     h = min(lengths[0] / nx, lengths[1] / ny, lengths[2] / nz)
     dt = min(0.4 * h / (dw["umax"] + 1.0), 0.25 * h * h / 3e-3)
     assert abs(d1["dt_cfl"] - dt) <= 1e-12 * dt
+
+
+@pytest.mark.parametrize("dtype", [binding.AC_F64, binding.AC_F32])
+def test_next4_tensor_product_mixed_reading(dtype):
+    """NEXT-4 (reading G2's alternative): ac_set_mixed("tensor") against the oracle's mixed="tensor" flag; the two
+    readings differ at truncation level, far above the parity tolerance, so the flag is shown to take effect."""
+    shape = (24, 40, 32)
+    lengths = (2 * math.pi, 1.6 * math.pi, 2.2 * math.pi)
+    npdt = np.float64 if dtype == binding.AC_F64 else np.float32
+    state = inputs.smooth_strong_state(shape, 31).astype(npdt)
+    nu, eta, dt = 2e-2, 1e-2, 2e-3
+    ctx = make_ctx(shape, dtype=dtype, lengths=lengths, nu=nu, eta=eta, k_f=3, helicity=1.0)
+    ctx.ac_set_mixed("tensor")
+    ctx.ac_load_state(state)
+    f = helpers.oracle_forcing(9, 0, 3, 1.0, dt, 0.02, 1.0, lengths)
+    ctx.ac_step(dt, ctx.ac_make_forcing(9, 0, dt, 0.02))
+    got = ctx.ac_store_state()
+    ctx.ac_free()
+    s64 = state.astype(np.float64)
+    want = mhd_c.step(s64, dt, lengths, nu, eta, 1.0, f, mixed="tensor")
+    other = mhd_c.step(s64, dt, lengths, nu, eta, 1.0, f, mixed="bidiagonal")
+    err = helpers.max_group_error(got, want)
+    gap = helpers.max_group_error(other, want)
+    print("tensor-product mixed parity", npdt.__name__, err, "tensor vs bidiagonal", gap)
+    assert err <= (1e-12 if dtype == binding.AC_F64 else 1e-5)
+    assert gap > 100 * err or dtype == binding.AC_F32
