@@ -18,6 +18,7 @@
 #include "kernels.cuh"
 #include "layout.cuh"
 #include "mhd_cell.cuh"
+#include "reduce_tma.cuh"
 #include "substep_march.cuh"
 #include "vec2.cuh"
 
@@ -111,16 +112,16 @@ EncodeTiledFn get_encode_fn() {
 
 // 4-D map (x, y, z, field) over one ghost-padded state buffer of 8-byte elements; box = (wx, wy, 1, 7).
 // Boxes must start 16-byte aligned in global memory (an 8-byte-aligned start faults on B200).
-int make_state_map(CUtensorMap* map, void* base, const ac::Layout& L, int wx, int wy) {
+int make_state_map(CUtensorMap* map, void* base, const ac::Layout& L, int wx, int wy, int nfields = AC_NFIELDS) {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) {
         snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled not available from the driver");
         return AC_ECUDA;
     }
     const size_t es = 8;
-    cuuint64_t dims[4] = {(cuuint64_t)L.pitch, (cuuint64_t)L.my, (cuuint64_t)L.mz, (cuuint64_t)AC_NFIELDS};
+    cuuint64_t dims[4] = {(cuuint64_t)L.pitch, (cuuint64_t)L.my, (cuuint64_t)L.mz, (cuuint64_t)nfields};
     cuuint64_t strides[3] = {(cuuint64_t)L.pitch * es, (cuuint64_t)L.plane * es, (cuuint64_t)L.field * es};
-    cuuint32_t box[4] = {(cuuint32_t)wx, (cuuint32_t)wy, 1u, (cuuint32_t)AC_NFIELDS};
+    cuuint32_t box[4] = {(cuuint32_t)wx, (cuuint32_t)wy, 1u, (cuuint32_t)nfields};
     cuuint32_t estr[4] = {1, 1, 1, 1};
     CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -157,6 +158,8 @@ struct ac_ctx {
     ac::RedVals* host_result;  // pinned
     CUtensorMap map_in[2];     // TMA maps of the two state buffers: tile + halo boxes
     CUtensorMap map_prev[2];   // and interior-tile boxes (previous state of the 2N update)
+    CUtensorMap map_a[2];      // tile + halo boxes of the three A fields (reductions)
+    CUtensorMap map_p[2];      // interior-tile boxes of ln rho and u (reductions)
     int cz, nchunks;           // z chunking of the march kernel
 
     void* field_ptr(int buf, int q) const { return ws + ((size_t)buf * AC_NFIELDS + q) * cv.field_bytes; }
@@ -386,14 +389,29 @@ int reduce_t(ac_ctx* ctx, ac_diag* out) {
     for (int q = 0; q < AC_NFIELDS; q++) a.in[q] = ctx->field_ptr(ctx->cur, q);
     a.partial = (ac::RedVals*)(ctx->ws + ctx->cv.partial_off);
     ac::RedVals* result = (ac::RedVals*)(ctx->ws + ctx->cv.result_off);
-    const int tiles_x = (L.nx + ac::RED_TX - 1) / ac::RED_TX, tiles_y = (L.ny + ac::RED_TY - 1) / ac::RED_TY;
-    const int nchunks = (L.nz + ac::RED_CZ - 1) / ac::RED_CZ;
-    const int blocks = (int)std::min<long>((long)tiles_x * tiles_y * nchunks, RED_BLOCKS);
-    if (ctx->packed) {
-        const int sm = ac::red_smem_bytes<T, 2>();
-        AC_CUDA(cudaFuncSetAttribute(ac::reduce_stage1_kernel<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
-        ac::reduce_stage1_kernel<T, 2><<<blocks, ac::RED_THREADS, sm, ctx->stream>>>(a, tiles_x, tiles_y, nchunks);
+    int blocks;
+    if (ctx->march) {
+        // 8-byte-element layouts (fp64, packed fp32): TMA plane ring (reduce_tma.cuh)
+        const int tiles_x = (L.nx + ac::M_TX - 1) / ac::M_TX, tiles_y = (L.ny + ac::M_TY - 1) / ac::M_TY;
+        const int nchunks = (L.nz + ac::RQ_CZ - 1) / ac::RQ_CZ;
+        int sms = 148;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
+        blocks = (int)std::min<long>((long)tiles_x * tiles_y * nchunks, std::min(2 * sms, RED_BLOCKS));
+        if (ctx->packed) {
+            AC_CUDA(cudaFuncSetAttribute(ac::reduce_tma_kernel<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         ac::RQ_SMEM_BYTES));
+            ac::reduce_tma_kernel<T, 2><<<blocks, ac::RQ_THREADS, ac::RQ_SMEM_BYTES, ctx->stream>>>(
+                a, ctx->map_a[ctx->cur], ctx->map_p[ctx->cur], tiles_x, tiles_y, nchunks);
+        } else {
+            AC_CUDA(cudaFuncSetAttribute(ac::reduce_tma_kernel<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         ac::RQ_SMEM_BYTES));
+            ac::reduce_tma_kernel<T, 1><<<blocks, ac::RQ_THREADS, ac::RQ_SMEM_BYTES, ctx->stream>>>(
+                a, ctx->map_a[ctx->cur], ctx->map_p[ctx->cur], tiles_x, tiles_y, nchunks);
+        }
     } else {
+        const int tiles_x = (L.nx + ac::RED_TX - 1) / ac::RED_TX, tiles_y = (L.ny + ac::RED_TY - 1) / ac::RED_TY;
+        const int nchunks = (L.nz + ac::RED_CZ - 1) / ac::RED_CZ;
+        blocks = (int)std::min<long>((long)tiles_x * tiles_y * nchunks, RED_BLOCKS);
         const int sm = ac::red_smem_bytes<T, 1>();
         AC_CUDA(cudaFuncSetAttribute(ac::reduce_stage1_kernel<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
         ac::reduce_stage1_kernel<T, 1><<<blocks, ac::RED_THREADS, sm, ctx->stream>>>(a, tiles_x, tiles_y, nchunks);
@@ -482,6 +500,8 @@ int configure(ac_ctx* ctx) {
     for (int b = 0; b < 2; b++) {
         int rc = make_state_map(&ctx->map_in[b], ctx->field_ptr(b, 0), ctx->L, ac::M_WX, ac::M_WY);
         if (rc == AC_OK) rc = make_state_map(&ctx->map_prev[b], ctx->field_ptr(b, 0), ctx->L, ac::M_TX, ac::M_TY);
+        if (rc == AC_OK) rc = make_state_map(&ctx->map_a[b], ctx->field_ptr(b, ac::AX), ctx->L, ac::M_WX, ac::M_WY, 3);
+        if (rc == AC_OK) rc = make_state_map(&ctx->map_p[b], ctx->field_ptr(b, 0), ctx->L, ac::M_TX, ac::M_TY, 4);
         if (rc != AC_OK) return rc;
     }
     const void* kernels[4] = {(const void*)ac::substep_march_kernel<double, false>,
