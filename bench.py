@@ -223,6 +223,16 @@ def run_ours(args):
         per = np.array([ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)])
         total_ms = max_over_ranks(total_ms, dist, "cuda")
         diag = ctx.ac_reduce()
+        # S9 (not part of the step): the reductions over the resident state, timed the same way
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        red_ms = []
+        for _ in range(5):
+            r0.record(ctx.stream)
+            ctx.ac_reduce()
+            r1.record(ctx.stream)
+            torch.cuda.synchronize()
+            red_ms.append(r0.elapsed_time(r1))
+        red_ms = float(np.median(red_ms))
         ms_per_step = total_ms / args.steps
         value = whole_job_value(n, world, ms_per_step)
         peak, peak_src = measured_peak()
@@ -233,6 +243,10 @@ def run_ours(args):
             "value": value, "ms_per_step": ms_per_step, "ms_median": float(np.median(per)),
             "ms_p90": float(np.percentile(per, 90)), "dt": dt, "launches": launches, "clocks": clocks,
             "diag": {k: diag[k] for k in ("urms", "brms", "nonfinite")},
+            "s9_reduce": {"ms": red_ms, "algorithmic_bytes": 7 * es * n ** 3,
+                          "achieved": 7 * es * n ** 3 / (red_ms * 1e-3) / 1e9, "unit": "GB/s",
+                          "frac": 7 * es * n ** 3 / (red_ms * 1e-3) / 1e9 / measured_peak()[0],
+                          "what": "ac_reduce (stage-1 + stage-2 kernels + 48-byte D2H), median of 5"},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": committed_traffic(dtype_name), "peak_source": peak_src,
                          "kernel": "substep (avg of the 3 launches of a step)",
@@ -293,12 +307,14 @@ def run_ours(args):
             "ms_median": main["ms_median"], "ms_p90": main["ms_p90"],
             "roofline": main["roofline"], "cpu_baseline": cpu, "e2e": main.get("e2e"),
             "gpu_launches": main["launches"], "clocks": main["clocks"], "diag": main["diag"],
+            "s9_reduce": main["s9_reduce"],
             "paper_context": {"astaroth_4xV100_fp64_cell_updates_per_s": 1.0 / 0.65e-9,
                               "pencil_40cores_cell_updates_per_s": 1.0 / 23.17e-9, "source": "PAPER.md:535"},
         }
         if other is not None:
             line["also"] = {"dtype": other_name, "value": other["value"], "ms_per_step": other["ms_per_step"],
                             "ms_median": other["ms_median"], "roofline": other["roofline"], "clocks": other["clocks"],
+                            "s9_reduce": other["s9_reduce"],
                             "gpu_launches": other["launches"]}
         print(json.dumps(line))
     if dist is not None:
