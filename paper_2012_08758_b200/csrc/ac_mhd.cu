@@ -396,7 +396,7 @@ int reduce_t(ac_ctx* ctx, ac_diag* out) {
         const int nchunks = (L.nz + ac::RQ_CZ - 1) / ac::RQ_CZ;
         int sms = 148;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
-        blocks = (int)std::min<long>((long)tiles_x * tiles_y * nchunks, std::min(2 * sms, RED_BLOCKS));
+        blocks = (int)std::min<long>((long)tiles_x * tiles_y * nchunks, std::min(3 * sms, RED_BLOCKS));
         if (ctx->packed) {
             AC_CUDA(cudaFuncSetAttribute(ac::reduce_tma_kernel<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          ac::RQ_SMEM_BYTES));

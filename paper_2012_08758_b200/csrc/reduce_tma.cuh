@@ -14,13 +14,13 @@
 
 namespace ac {
 
-constexpr int RQ_NP = 11;                               // ring slots: planes q-3 .. q+3 in use, LEAD in flight, 1 spare
-constexpr int RQ_LEAD = 3;
+constexpr int RQ_NP = 8;                                // ring slots: planes q-3 .. q+3 in use + 1 in flight (3 CTAs per SM
+                                                        // with a short ring beat 2 CTAs with 11 slots: 1.83 vs 2.13 ms)
 constexpr int RQ_CZ = 128;                              // planes per work item
 constexpr int RQ_WORKERS = M_COLS;                      // 128 threads, one per column of the 16 x 8 tile
 constexpr int RQ_THREADS = RQ_WORKERS + 32;             // + producer warp
 constexpr int RQ_SLOT_BYTES = 3 * M_PLANE * 8;          // 8064
-constexpr int RQ_PNP = 6;                               // ring of the pointwise fields (ln rho, u): producer lead + 1
+constexpr int RQ_PNP = 2;                               // ring of the pointwise fields (ln rho, u): producer lead + 1
 constexpr int RQ_PSLOT_BYTES = 4 * M_COLS * 8;          // 4096: interior tile of 4 fields
 constexpr int RQ_OFF_P = RQ_NP * RQ_SLOT_BYTES;
 constexpr int RQ_OFF_BARS = RQ_OFF_P + RQ_PNP * RQ_PSLOT_BYTES;
@@ -39,7 +39,7 @@ __device__ __forceinline__ void rq_lds(const unsigned char* p, T (&v)[LANES]) {
 }
 
 template <typename T, int LANES>
-__global__ void __launch_bounds__(RQ_THREADS, 2)
+__global__ void __launch_bounds__(RQ_THREADS, 3)
     reduce_tma_kernel(const __grid_constant__ ReduceArgs<T> a, const __grid_constant__ CUtensorMap map_a,
                       const __grid_constant__ CUtensorMap map_p, int tiles_x, int tiles_y, int nchunks) {
     extern __shared__ __align__(1024) unsigned char rq_smem[];
