@@ -333,11 +333,10 @@ int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
             ctx->launches++;
             // S1: refresh the ghost zones of the buffer just written
             const int nb_rows = 2 * ac::R * L.my + 2 * ac::R * L.nz;
-            const int xb = (L.nx + 2 * ac::R + ac::M_GHOST_THREADS - 1) / ac::M_GHOST_THREADS;
-            const long na = ((long)L.ny * L.nz * 8 + ac::M_GHOST_THREADS - 1) / ac::M_GHOST_THREADS;
-            dim3 gg((unsigned)((long)nb_rows * xb + na), AC_NFIELDS, 1);
+            const int na_tasks = (int)(((long)L.ny * L.nz + ac::M_GHOST_ROWS_PER_TASK - 1) / ac::M_GHOST_ROWS_PER_TASK);
+            dim3 gg((unsigned)std::min(nb_rows + na_tasks, RED_BLOCKS), AC_NFIELDS, 1);
             ac::ghost_fill_kernel<E><<<gg, ac::M_GHOST_THREADS, 0, ctx->stream>>>((E*)ctx->field_ptr(1 - ctx->cur, 0), L,
-                                                                              nb_rows, xb);
+                                                                              nb_rows, na_tasks);
             ctx->launches++;
             ctx->cur = 1 - ctx->cur;
         }

@@ -215,46 +215,52 @@ __device__ __forceinline__ E m_mixxy(const E* p, const E (&cm)[3]) {
 
 // S1, periodic ghost zones of one state buffer after a substep (the paper's "local boundary
 // transfer"; wrap of PAPER.md:111).  Every ghost cell copies its periodic source
-// cell, which is always an interior cell, so the order of the copies does not matter.  Blocks
-// [0, nb_rows * xb) serve the rows that are ghosts in y or z (whole rows, x ghosts included),
-// the remaining blocks the 2 x 3 x-ghost cells of the interior rows.  z images of packed fp32
+// cell, which is always an interior cell, so the order of the copies does not matter.  Tasks
+// [0, nb_rows) are the rows that are ghosts in y or z (whole rows, x ghosts included), the remaining
+// tasks the 2 x 3 x-ghost cells of 42 interior rows each; blocks take tasks round-robin.  z images of packed fp32
 // pairs swap lanes (cell z - nz/2 of the pair below is cell z + nz/2 of the periodic domain).
-constexpr int M_GHOST_THREADS = 128;
+constexpr int M_GHOST_THREADS = 256;
+constexpr int M_GHOST_ROWS_PER_TASK = M_GHOST_THREADS / (2 * R);   // interior rows whose 6 x ghosts one task copies
 template <typename E>
-__global__ void __launch_bounds__(M_GHOST_THREADS) ghost_fill_kernel(E* __restrict__ base, Layout L, int nb_rows, int xb) {
+__global__ void __launch_bounds__(M_GHOST_THREADS) ghost_fill_kernel(E* __restrict__ base, Layout L, int nb_rows, int na_tasks) {
     E* __restrict__ f = base + (size_t)blockIdx.y * L.field;
-    const long b = blockIdx.x;
-    const long nb = (long)nb_rows * xb;
-    if (b < nb) {
-        const int row = (int)(b / xb);
-        const int x = (int)(b % xb) * M_GHOST_THREADS + (int)threadIdx.x - R;
-        if (x >= L.nx + R) return;
-        int y, z;
-        if (row < 2 * R * L.my) {            // the 6 ghost planes, all rows
-            const int zi = row / L.my;
-            z = zi < R ? zi - R : L.nz + zi - R;
-            y = row % L.my - R;
-        } else {                             // the 6 ghost rows of every interior plane
-            const int r2 = row - 2 * R * L.my;
-            const int yi = r2 % (2 * R);
-            z = r2 / (2 * R);
-            y = yi < R ? yi - R : L.ny + yi - R;
+    const int tid = threadIdx.x;
+    for (int task = blockIdx.x; task < nb_rows + na_tasks; task += gridDim.x) {
+        if (task < nb_rows) {
+            // one ghost row (ghost in y or z), whole: x ghosts included
+            const int row = task;
+            int y, z;
+            if (row < 2 * R * L.my) {            // the 6 ghost planes, all rows
+                const int zi = row / L.my;
+                z = zi < R ? zi - R : L.nz + zi - R;
+                y = row % L.my - R;
+            } else {                             // the 6 ghost rows of every interior plane
+                const int r2 = row - 2 * R * L.my;
+                const int yi = r2 % (2 * R);
+                z = r2 / (2 * R);
+                y = yi < R ? yi - R : L.ny + yi - R;
+            }
+            const int ys = y < 0 ? y + L.ny : (y >= L.ny ? y - L.ny : y);
+            const int zs = z < 0 ? z + L.nz : (z >= L.nz ? z - L.nz : z);
+            const E* __restrict__ src = f + L.idx(0, ys, zs);
+            E* __restrict__ dst = f + L.idx(0, y, z);
+            for (int x = tid - R; x < L.nx + R; x += M_GHOST_THREADS) {
+                const int xs = x < 0 ? x + L.nx : (x >= L.nx ? x - L.nx : x);
+                E v = src[xs];
+                if (zs != z) v = vswap(v);
+                dst[x] = v;
+            }
+        } else {
+            // the 2 x 3 x-ghost cells of M_GHOST_ROWS_PER_TASK interior rows
+            const long r = (long)(task - nb_rows) * M_GHOST_ROWS_PER_TASK + tid / (2 * R);
+            const int j = tid % (2 * R);
+            if (tid < M_GHOST_ROWS_PER_TASK * 2 * R && r < (long)L.ny * L.nz) {
+                const int y = (int)(r % L.ny), z = (int)(r / L.ny);
+                const int x = j < R ? j - R : L.nx + j - R;
+                const int xs = j < R ? x + L.nx : x - L.nx;
+                f[L.idx(x, y, z)] = f[L.idx(xs, y, z)];
+            }
         }
-        const int xs = x < 0 ? x + L.nx : (x >= L.nx ? x - L.nx : x);
-        const int ys = y < 0 ? y + L.ny : (y >= L.ny ? y - L.ny : y);
-        const int zs = z < 0 ? z + L.nz : (z >= L.nz ? z - L.nz : z);
-        E v = f[L.idx(xs, ys, zs)];
-        if (zs != z) v = vswap(v);
-        f[L.idx(x, y, z)] = v;
-    } else {
-        const long t = (b - nb) * M_GHOST_THREADS + threadIdx.x;
-        const int j = (int)(t & 7);
-        const long r = t >> 3;
-        if (j >= 2 * R || r >= (long)L.ny * L.nz) return;
-        const int y = (int)(r % L.ny), z = (int)(r / L.ny);
-        const int x = j < R ? j - R : L.nx + j - R;
-        const int xs = j < R ? x + L.nx : x - L.nx;
-        f[L.idx(x, y, z)] = f[L.idx(xs, y, z)];
     }
 }
 
