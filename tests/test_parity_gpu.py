@@ -405,3 +405,46 @@ def test_next4_tensor_product_mixed_reading(dtype):
     print("tensor-product mixed parity", npdt.__name__, err, "tensor vs bidiagonal", gap)
     assert err <= (1e-12 if dtype == binding.AC_F64 else 1e-5)
     assert gap > 100 * err or dtype == binding.AC_F32
+
+
+def test_per_field_load_store_and_option_errors():
+    """ac_load_field / ac_store_field: the context counts as loaded only after all 7 fields; results equal the
+    whole-state calls; bad arguments are refused; ac_set_mixed / ac_set_variant drop a loaded state."""
+    import torch
+    shape = (16, 24, 32)
+    state = inputs.gaussian_state(shape, 8, u_amp=1e-2, a_amp=1e-3)
+    ctx = make_ctx(shape, nu=1e-2, eta=1e-2)
+    out = np.empty(shape)
+    for q in range(7):
+        with pytest.raises(binding.AcError):
+            ctx.ac_store_field(q, out)                     # AC_ESTATE: not all fields loaded yet
+        with pytest.raises(binding.AcError):
+            ctx.ac_step(1e-3, None)
+        if q % 2:
+            ctx.ac_load_field(q, torch.from_numpy(state[q]).cuda())
+        else:
+            ctx.ac_load_field(q, np.ascontiguousarray(state[q]))
+    for bad_q in (-1, 7):
+        with pytest.raises(binding.AcError):
+            ctx._lib and binding._check(ctx._lib.ac_load_field(ctx._ctx, bad_q, out.ctypes.data, 0), "ac_load_field")
+    got = np.stack([ctx.ac_store_field(q, np.empty(shape)) for q in range(7)])
+    assert np.array_equal(got, state)
+    ctx.ac_step(1e-3, None)
+    a = ctx.ac_store_state()
+    ctx2 = make_ctx(shape, nu=1e-2, eta=1e-2)
+    ctx2.ac_load_state(state)
+    ctx2.ac_step(1e-3, None)
+    assert np.array_equal(a, ctx2.ac_store_state())
+    dev = torch.empty(shape, dtype=torch.float64, device="cuda")
+    ctx2.ac_store_field(3, dev)
+    ctx2.synchronize()
+    assert np.array_equal(dev.cpu().numpy(), a[3])
+    with pytest.raises(binding.AcError):
+        ctx2.ac_set_mixed(2)
+    with pytest.raises(binding.AcError):
+        ctx2.ac_set_variant(5)
+    ctx2.ac_set_mixed("tensor")                            # reconfigures: the loaded state is gone
+    with pytest.raises(binding.AcError):
+        ctx2.ac_step(1e-3, None)
+    ctx.ac_free()
+    ctx2.ac_free()
