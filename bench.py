@@ -292,8 +292,18 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n_s = min(n, args.ref_sample)
         v, sec, cores = time_oracle(n_s, cfg, 1)
-        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "ns_per_cell_step": 1e9 / v,
                "sample": "1 RK3 step of the C oracle (fp64, OpenMP) on a %d^3 box of the same recipe; %.1f s" % (n_s, sec)}
+        # the same oracle on one thread, on a 64^3 box to keep the run short
+        from oracle import mhd_c
+        nthreads = mhd_c.max_threads()
+        mhd_c.set_threads(1)
+        try:
+            v1, sec1, _ = time_oracle(min(n_s, 64), cfg, 1)
+        finally:
+            mhd_c.set_threads(nthreads)
+        cpu["one_thread"] = {"value": v1, "unit": UNIT, "ns_per_cell_step": 1e9 / v1,
+                             "sample": "1 step on a %d^3 box, 1 thread; %.1f s" % (min(n_s, 64), sec1)}
 
     if rank == 0:
         line = {
