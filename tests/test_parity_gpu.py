@@ -272,7 +272,8 @@ def test_config2_full_grid_ten_steps_with_logged_diagnostics():
     assert log[-1][0] > log[0][0]                         # the forcing is stirring the flow
 
 
-def test_p16_periodic_replication_1024cubed_fp64():
+@pytest.mark.parametrize("dtype", [binding.AC_F64, binding.AC_F32])
+def test_p16_periodic_replication_1024cubed(dtype):
     """P16, BASELINE config 5 size: a 128^3 state tiled 8 x per axis on a 1024^3
     grid (box 2 pi) must evolve exactly like the 128^3 state in a box of side 2 pi / 8, which is
     all the oracle ever runs.  Forcing wavevector (8, 16, -8): a multiple of 8 per axis, so the
@@ -280,7 +281,12 @@ def test_p16_periodic_replication_1024cubed_fp64():
     Fields are streamed through ac_load_field / ac_store_field (8.6 GB each)."""
     import torch
     n, t, rep = 1024, 128, 8
-    need = binding.ac_workspace_bytes((n, n, n), TWO_PI3, binding.AC_F64) + 3 * 8 * n ** 3
+    f64 = dtype == binding.AC_F64
+    tdt = torch.float64 if f64 else torch.float32
+    need = binding.ac_workspace_bytes((n, n, n), TWO_PI3, dtype) + 3 * (8 if f64 else 4) * n ** 3
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()                               # give back what earlier tests' contexts cached
     free, _total = torch.cuda.mem_get_info()
     if free < need:
         pytest.skip("needs %.0f GB of free device memory" % (need / 1e9))
@@ -292,34 +298,37 @@ def test_p16_periodic_replication_1024cubed_fp64():
     h = 2 * math.pi / n
     dt = 0.4 * h / (float(np.sqrt((tile[1:4] ** 2).sum(axis=0).max())) + 1.0)
     forcing = ((8.0, 16.0, -8.0), 0.3, (0.5, -0.25, 0.125), (0.1, 0.2, 0.5))
+    if not f64:
+        tile = tile.astype(np.float32).astype(np.float64)     # the oracle starts from the fp32-rounded inputs (G14)
     want = helpers.oracle_run(tile, 1, dt, small, nu, nu, 1.0, lambda s: forcing)[0]
 
-    ctx = make_ctx((n, n, n), nu=nu, eta=nu, k_f=3, helicity=0.0)
+    ctx = make_ctx((n, n, n), dtype=dtype, nu=nu, eta=nu, k_f=3, helicity=0.0)
     for q in range(7):
-        dev = torch.from_numpy(tile[q]).cuda().repeat(rep, rep, rep).contiguous()
+        dev = torch.from_numpy(tile[q]).to(tdt).cuda().repeat(rep, rep, rep).contiguous()
         ctx.ac_load_field(q, dev)
         ctx.synchronize()
         del dev
     d0 = ctx.ac_reduce()
     dwant = mhd_c.diagnostics(tile, small)
-    assert abs(d0["urms"] - dwant["urms"]) <= 1e-12 * dwant["urms"]
-    assert abs(d0["bmax"] - dwant["bmax"]) <= 1e-11 * dwant["bmax"]
+    assert abs(d0["urms"] - dwant["urms"]) <= (1e-12 if f64 else 1e-6) * dwant["urms"]
+    assert abs(d0["bmax"] - dwant["bmax"]) <= (1e-11 if f64 else 1e-4) * dwant["bmax"]
     ctx.ac_step(dt, forcing)
-    out = torch.empty((n, n, n), dtype=torch.float64, device="cuda")
+    out = torch.empty((n, n, n), dtype=tdt, device="cuda")
     s_u, s_a = np.abs(want[1:4]).max(), np.abs(want[4:7]).max()
     scale = [max(np.abs(want[0]).max(), s_u), s_u, s_u, s_u, s_a, s_a, s_a]
     worst = 0.0
     for q in range(7):
         ctx.ac_store_field(q, out)
         ctx.synchronize()
-        ref = torch.from_numpy(want[q]).cuda()
+        ref = torch.from_numpy(want[q]).to(tdt).cuda()
         # every one of the 512 tiles against the oracle field
         blocks = out.view(rep, t, rep, t, rep, t)
         err = (blocks - ref.view(1, t, 1, t, 1, t)).abs().max().item()
         worst = max(worst, err / scale[q])
     ctx.ac_free()
+    del ctx, out, ref, blocks
     print("P16 worst group-scaled error", worst)
-    assert worst <= 1e-12
+    assert worst <= (1e-12 if f64 else 1e-5)
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
