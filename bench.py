@@ -250,6 +250,8 @@ def run_ours(args):
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": committed_traffic(dtype_name), "peak_source": peak_src,
                          "kernel": "substep (avg of the 3 launches of a step)",
+                         "note": "reported against HBM as BASELINE.json's metric asks; the kernel itself is limited by "
+                                 "the shared-memory data pipe (81 % of peak, profiles/r01d_march.md) and the 1000 W power cap",
                          "algorithmic_bytes_per_launch": alg_bytes_launch},
         }
         if do_e2e:
