@@ -3,10 +3,12 @@
 //
 // B needs six first derivatives of A (36 neighbours, radius 3).  The three A fields are streamed plane by
 // plane through a shared-memory ring by TMA (one 4-D box of tile + halo x 3 fields per plane, issued by a
-// producer warp LEAD planes ahead); a worker thread owns one (x, y) column, and when plane q + 3 has landed it
-// gathers the 36 neighbours of cell (x, y, q) from the ring, so no derivative state is carried in registers
-// and the loads never wait on DRAM.  ln rho and u of the plane being finished arrive by a second, interior-only
-// TMA box in a small ring of their own.  A CTA takes (tile, z chunk) work items round-robin (fixed assignment: deterministic) and leaves one
+// producer warp up to 3 planes ahead), ln rho and u by a second, interior-only box; the loads never wait on
+// DRAM.  A worker thread owns one (x, y) column: from the plane that has just landed it takes the pointwise
+// fields, the 24 in-plane neighbours (d_x, d_y of A_z, d_x A_y, d_y A_x) and the centre values of A_x, A_y; the z
+// derivatives come from a 7-plane register history of those centre values and the in-plane parts of B wait
+// 3 planes in registers (31 shared-memory loads per cell; gathering the z neighbours from a longer ring took
+// 43 and an 8-slot ring: 1.83 ms against 1.43 ms for this version at 512^3 fp64).  A CTA takes (tile, z chunk) work items round-robin (fixed assignment: deterministic) and leaves one
 // partial; reduce_stage2_kernel folds the partials in a fixed order.
 #pragma once
 #include "kernels.cuh"
@@ -14,16 +16,14 @@
 
 namespace ac {
 
-constexpr int RQ_NP = 8;                                // ring slots: planes q-3 .. q+3 in use + 1 in flight (3 CTAs per SM
-                                                        // with a short ring beat 2 CTAs with 11 slots: 1.83 vs 2.13 ms)
+constexpr int RQ_NP = 4;                                // ring slots: the plane being visited + 3 in flight
 constexpr int RQ_CZ = 128;                              // planes per work item
 constexpr int RQ_WORKERS = M_COLS;                      // 128 threads, one per column of the 16 x 8 tile
 constexpr int RQ_THREADS = RQ_WORKERS + 32;             // + producer warp
-constexpr int RQ_SLOT_BYTES = 3 * M_PLANE * 8;          // 8064
-constexpr int RQ_PNP = 2;                               // ring of the pointwise fields (ln rho, u): producer lead + 1
-constexpr int RQ_PSLOT_BYTES = 4 * M_COLS * 8;          // 4096: interior tile of 4 fields
+constexpr int RQ_SLOT_BYTES = 3 * M_PLANE * 8;          // 8064: A_x, A_y, A_z, tile + halo
+constexpr int RQ_PSLOT_BYTES = 4 * M_COLS * 8;          // 4096: ln rho, u, interior tile
 constexpr int RQ_OFF_P = RQ_NP * RQ_SLOT_BYTES;
-constexpr int RQ_OFF_BARS = RQ_OFF_P + RQ_PNP * RQ_PSLOT_BYTES;
+constexpr int RQ_OFF_BARS = RQ_OFF_P + RQ_NP * RQ_PSLOT_BYTES;
 constexpr int RQ_SMEM_BYTES = RQ_OFF_BARS + 2 * RQ_NP * 8;
 static_assert(RQ_SLOT_BYTES % 128 == 0, "TMA destinations must stay 128-byte aligned");
 
@@ -66,16 +66,16 @@ __global__ void __launch_bounds__(RQ_THREADS, 3)
             const int zs = (int)(w / ((long)tiles_x * tiles_y)) * RQ_CZ;
             const int niter = min(zs + RQ_CZ, L.nz) - zs + 2 * R;
             for (int k = 0; k < niter; k++, issued++) {
-                // the slot of plane `issued` was last read 7 planes after the plane it held (issued - NP)
-                const long need = issued - RQ_NP + 2 * R;
+                // a slot is read only in the iteration its plane arrives in
+                const long need = issued - RQ_NP;
                 if (need >= 0) m_bar_wait<100>(&done[need % RQ_NP], (uint32_t)((need / RQ_NP) & 1));
                 const int slot = (int)(issued % RQ_NP);
-                const bool fin = k >= 2 * R;        // plane zs + k - 6 is finished in this iteration: bring its ln rho, u
-                m_bar_expect_tx(&full[slot], (uint32_t)(RQ_SLOT_BYTES + (fin ? RQ_PSLOT_BYTES : 0)));
+                const bool inner = k >= R && k < niter - R;     // plane zs - 3 + k is one of the item's own: bring ln rho, u
+                m_bar_expect_tx(&full[slot], (uint32_t)(RQ_SLOT_BYTES + (inner ? RQ_PSLOT_BYTES : 0)));
                 m_tma_load_4d(rq_smem + slot * RQ_SLOT_BYTES, &map_a, &full[slot], x0 - M_HX + L.gx, y0, zs + k, 0);
-                if (fin)
-                    m_tma_load_4d(rq_smem + RQ_OFF_P + (int)(issued % RQ_PNP) * RQ_PSLOT_BYTES, &map_p, &full[slot],
-                                  x0 + L.gx, y0 + R, zs + k - R, 0);
+                if (inner)
+                    m_tma_load_4d(rq_smem + RQ_OFF_P + slot * RQ_PSLOT_BYTES, &map_p, &full[slot], x0 + L.gx, y0 + R, zs + k,
+                                  0);
             }
         }
         return;
@@ -92,20 +92,40 @@ __global__ void __launch_bounds__(RQ_THREADS, 3)
         const int ze = min(zs + RQ_CZ, L.nz);
         const int niter = ze - zs + 2 * R;
         const bool valid = x < L.nx && y < L.ny;
+        T hax[7][LANES], hay[7][LANES];                               // A_x, A_y of planes p-6 .. p (this column)
+        T pbx[4][LANES], pby[4][LANES], pbz[4][LANES];                // d_y A_z, d_x A_z, B_z of planes p-3 .. p
+#pragma unroll
+        for (int r = 0; r < 7; r++)
+#pragma unroll
+            for (int i = 0; i < LANES; i++) hax[r][i] = hay[r][i] = T(0);
+#pragma unroll
+        for (int r = 0; r < 4; r++)
+#pragma unroll
+            for (int i = 0; i < LANES; i++) pbx[r][i] = pby[r][i] = pbz[r][i] = T(0);
+#pragma unroll 1
         for (int k = 0; k < niter; k++, it++) {
-            const bool fin = k >= 2 * R;
-            m_bar_wait<0>(&full[it % RQ_NP], (uint32_t)((it / RQ_NP) & 1));
-            if (fin && valid) {
-                T ux[LANES], uy[LANES], uz[LANES], l[LANES];
-                const unsigned char* pp = rq_smem + RQ_OFF_P + (int)(it % RQ_PNP) * RQ_PSLOT_BYTES + tid * 8;
-                rq_lds<T, LANES>(pp, l);
-                rq_lds<T, LANES>(pp + M_COLS * 8, ux);
-                rq_lds<T, LANES>(pp + 2 * M_COLS * 8, uy);
-                rq_lds<T, LANES>(pp + 3 * M_COLS * 8, uz);
-                // plane q + j sits in the slot of running index it - 3 + j
-                auto plane = [&](int j) { return rq_smem + (int)((it - R + j) % RQ_NP) * RQ_SLOT_BYTES + cell_off; };
-                const unsigned char* p0 = plane(0);
-                // first derivative of A field f (0, 1, 2) along x (stride 8 B) or y (stride M_WX * 8 B) in plane q
+            const int slot = (int)(it % RQ_NP);
+#pragma unroll
+            for (int r = 0; r < 6; r++)
+#pragma unroll
+                for (int i = 0; i < LANES; i++) {
+                    hax[r][i] = hax[r + 1][i];
+                    hay[r][i] = hay[r + 1][i];
+                }
+#pragma unroll
+            for (int r = 0; r < 3; r++)
+#pragma unroll
+                for (int i = 0; i < LANES; i++) {
+                    pbx[r][i] = pbx[r + 1][i];
+                    pby[r][i] = pby[r + 1][i];
+                    pbz[r][i] = pbz[r + 1][i];
+                }
+            m_bar_wait<0>(&full[slot], (uint32_t)((it / RQ_NP) & 1));
+            const unsigned char* p0 = rq_smem + slot * RQ_SLOT_BYTES + cell_off;
+            rq_lds<T, LANES>(p0, hax[6]);
+            rq_lds<T, LANES>(p0 + M_PLANE * 8, hay[6]);
+            if (k >= R && k < niter - R && valid) {
+                // the plane is one of the item's own: in-plane parts of B, and the pointwise fields
                 auto din = [&](int f, int stride, int axis, T (&r)[LANES]) {
                     const unsigned char* p = p0 + f * (M_PLANE * 8);
                     T r_[LANES];
@@ -121,52 +141,52 @@ __global__ void __launch_bounds__(RQ_THREADS, 3)
 #pragma unroll
                     for (int i = 0; i < LANES; i++) r[i] = r_[i];
                 };
-                // and along z: the same column of planes q -+ m
-                auto dz = [&](int f, T (&r)[LANES]) {
-                    T r_[LANES];
-#pragma unroll
-                    for (int m = 1; m <= 3; m++) {
-                        T pp[LANES], mm[LANES];
-                        rq_lds<T, LANES>(plane(m) + f * (M_PLANE * 8), pp);
-                        rq_lds<T, LANES>(plane(-m) + f * (M_PLANE * 8), mm);
-#pragma unroll
-                        for (int i = 0; i < LANES; i++)
-                            r_[i] = (m == 1) ? a.c1[2][0] * (pp[i] - mm[i]) : fma_<T>(a.c1[2][m - 1], pp[i] - mm[i], r_[i]);
-                    }
-#pragma unroll
-                    for (int i = 0; i < LANES; i++) r[i] = r_[i];
-                };
-                T azy[LANES], ayz[LANES], axz[LANES], azx[LANES], ayx[LANES], axy[LANES];
-                T ax[LANES], ay[LANES], az[LANES];
+                T azy[LANES], azx[LANES], ayx[LANES], axy[LANES], az[LANES];
+                T ux[LANES], uy[LANES], uz[LANES], l[LANES];
                 din(2, M_WX * 8, 1, azy);
-                dz(1, ayz);
-                dz(0, axz);
                 din(2, 8, 0, azx);
                 din(1, 8, 0, ayx);
                 din(0, M_WX * 8, 1, axy);
-                rq_lds<T, LANES>(p0, ax);
-                rq_lds<T, LANES>(p0 + M_PLANE * 8, ay);
                 rq_lds<T, LANES>(p0 + 2 * M_PLANE * 8, az);
+                const unsigned char* pp = rq_smem + RQ_OFF_P + slot * RQ_PSLOT_BYTES + tid * 8;
+                rq_lds<T, LANES>(pp, l);
+                rq_lds<T, LANES>(pp + M_COLS * 8, ux);
+                rq_lds<T, LANES>(pp + 2 * M_COLS * 8, uy);
+                rq_lds<T, LANES>(pp + 3 * M_COLS * 8, uz);
 #pragma unroll
                 for (int i = 0; i < LANES; i++) {
-                    const T bx = azy[i] - ayz[i] + a.bext[0];
-                    const T by = axz[i] - azx[i] + a.bext[1];
-                    const T bz = ayx[i] - axy[i] + a.bext[2];
+                    pbx[3][i] = azy[i];
+                    pby[3][i] = azx[i];
+                    pbz[3][i] = ayx[i] - axy[i] + a.bext[2];
                     const double u2 = (double)ux[i] * ux[i] + (double)uy[i] * uy[i] + (double)uz[i] * uz[i];
-                    const double b2 = (double)bx * bx + (double)by * by + (double)bz * bz;
                     acc.su += u2;
-                    acc.sb += b2;
                     acc.mu = fmax(acc.mu, u2);
-                    acc.mb = fmax(acc.mb, b2);
                     acc.lmin = fmin(acc.lmin, (double)l[i]);
                     acc.lmax = fmax(acc.lmax, (double)l[i]);
                     // a non-finite ln rho or A would hide in fmin/fmax: fold it into the sums
-                    const double chk = (double)l[i] + (double)ax[i] + (double)ay[i] + (double)az[i];
+                    const double chk = (double)l[i] + (double)hax[6][i] + (double)hay[6][i] + (double)az[i];
                     if (!isfinite(chk)) acc.su += chk;
                 }
             }
+            if (k >= 2 * R && valid) {                                // plane p - 3 has its 7-plane history: finish B there
+#pragma unroll
+                for (int i = 0; i < LANES; i++) {
+                    T ayz = a.c1[2][0] * (hay[4][i] - hay[2][i]);
+                    ayz = fma_<T>(a.c1[2][1], hay[5][i] - hay[1][i], ayz);
+                    ayz = fma_<T>(a.c1[2][2], hay[6][i] - hay[0][i], ayz);
+                    T axz = a.c1[2][0] * (hax[4][i] - hax[2][i]);
+                    axz = fma_<T>(a.c1[2][1], hax[5][i] - hax[1][i], axz);
+                    axz = fma_<T>(a.c1[2][2], hax[6][i] - hax[0][i], axz);
+                    const T bx = pbx[0][i] - ayz + a.bext[0];
+                    const T by = axz - pby[0][i] + a.bext[1];
+                    const T bz = pbz[0][i];
+                    const double b2 = (double)bx * bx + (double)by * by + (double)bz * bz;
+                    acc.sb += b2;
+                    acc.mb = fmax(acc.mb, b2);
+                }
+            }
             __syncwarp();
-            if (lane == 0) m_bar_arrive(&done[it % RQ_NP]);
+            if (lane == 0) m_bar_arrive(&done[slot]);
         }
     }
     // fold the 4 worker warps (the producer warp has left: no __syncthreads here)
