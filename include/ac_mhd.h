@@ -119,6 +119,32 @@ int ac_store_field(ac_ctx* ctx, int q, void* field, int dst_on_device);
  * Errors: AC_EINVAL (dt <= 0 or non-finite), AC_ESTATE, AC_ECUDA. */
 int ac_step(ac_ctx* ctx, double dt, const ac_forcing* forcing);
 
+/* ---- building blocks of a z-slab decomposition over several GPUs --------------------
+ * A rank owns nz_local planes of the global grid (its ac_grid carries nz = nz_local and lz = its share of the box)
+ * and the usual 3 ghost planes per side.  Between substeps the ghost planes must hold the neighbour ranks' boundary
+ * planes instead of the rank's own periodic images: the caller runs ONE substep with ac_substep (which also refreshes
+ * the x / y ghost zones and, harmlessly, writes the local periodic images into the z ghost planes), then overwrites
+ * the z ghost planes of every field of the current state with the neighbours' planes.  In the padded layout
+ * (ac_state_layout; element (x, y, z) of field q at ac_field_device_ptr(ctx, q) + (x + gx) + pitch * (y + 3) +
+ * plane_elems * (z + 3) elements) the planes to send, [nz_local, nz_local + 3) upwards and [3, 6) downwards, and the
+ * planes to receive, [0, 3) and [nz_local + 3, nz_local + 6), are contiguous blocks of 3 * plane_elems elements per
+ * field, so the exchange is 2 x 7 plain copies (peer copies, ncclSend/ncclRecv, torch.distributed) and needs no
+ * pack kernel.  The forcing phase of a rank is the global phase + k_z * z0 with z0 the position of its first plane.
+ * Only layouts with packed_pairs == 0 can be exchanged this way (fp64, or fp32 with ac_set_variant(ctx, 1)).
+ * ac_substep: substep s = 0, 1, 2 of the 2N-RK3 step; three calls with the same dt and forcing equal ac_step.
+ * ac_reduce_raw: the unnormalised reductions of this rank's cells, out = {sum |u|^2, max |u|^2, sum |B|^2, max |B|^2,
+ * min ln rho, max ln rho}, to be combined across ranks (sum, max, sum, max, min, max).  Synchronises the stream. */
+typedef struct {
+    int elem_bytes;          /* 8: double or packed fp32 pair; 4: plain float */
+    int packed_pairs;        /* 1: an element holds cells z and z + nz/2 (fp32 default variant) */
+    int gx, pitch, my, mz;   /* x ghost offset, row pitch, padded rows and planes, in elements */
+    size_t plane_elems, field_elems;
+} ac_layout_info;
+int ac_substep(ac_ctx* ctx, int s, double dt, const ac_forcing* forcing);
+int ac_state_layout(const ac_ctx* ctx, ac_layout_info* out);
+void* ac_field_device_ptr(ac_ctx* ctx, int q);
+int ac_reduce_raw(ac_ctx* ctx, double out[6]);
+
 /* rms/max reductions of |u| and |B| and min/max of ln rho over the current state, and the CFL
  * time step dt = min(C_u h/(umax + cs), C_nu h^2/max(nu, eta)) (G15).  Deterministic (fixed
  * two-stage tree, no floating-point atomics).  Synchronises the stream. */

@@ -18,7 +18,7 @@ EXPORTS = (
     "ac_workspace_bytes", "ac_init", "ac_load_state", "ac_store_state", "ac_load_field", "ac_store_field", "ac_step",
     "ac_reduce",
     "ac_forcing_from_draws", "ac_forcing_params", "ac_make_forcing", "ac_set_bext", "ac_set_cfl", "ac_set_variant",
-    "ac_set_upwind", "ac_set_mixed",
+    "ac_set_upwind", "ac_set_mixed", "ac_substep", "ac_state_layout", "ac_field_device_ptr", "ac_reduce_raw",
     "ac_launch_count", "ac_free", "ac_strerror", "ac_version",
 )
 
@@ -26,6 +26,12 @@ EXPORTS = (
 class AcGrid(ctypes.Structure):
     _fields_ = [("nx", ctypes.c_int), ("ny", ctypes.c_int), ("nz", ctypes.c_int),
                 ("lx", ctypes.c_double), ("ly", ctypes.c_double), ("lz", ctypes.c_double)]
+
+
+class AcLayoutInfo(ctypes.Structure):
+    _fields_ = [("elem_bytes", ctypes.c_int), ("packed_pairs", ctypes.c_int), ("gx", ctypes.c_int),
+                ("pitch", ctypes.c_int), ("my", ctypes.c_int), ("mz", ctypes.c_int),
+                ("plane_elems", ctypes.c_size_t), ("field_elems", ctypes.c_size_t)]
 
 
 class AcForcing(ctypes.Structure):
@@ -92,6 +98,14 @@ def load_library():
     L.ac_set_upwind.restype = i32
     L.ac_set_mixed.argtypes = [vp, i32]
     L.ac_set_mixed.restype = i32
+    L.ac_substep.argtypes = [vp, i32, dbl, ctypes.POINTER(AcForcing)]
+    L.ac_substep.restype = i32
+    L.ac_state_layout.argtypes = [vp, ctypes.POINTER(AcLayoutInfo)]
+    L.ac_state_layout.restype = i32
+    L.ac_field_device_ptr.argtypes = [vp, i32]
+    L.ac_field_device_ptr.restype = ctypes.c_void_p
+    L.ac_reduce_raw.argtypes = [vp, ctypes.POINTER(dbl)]
+    L.ac_reduce_raw.restype = i32
     L.ac_launch_count.argtypes = [vp]
     L.ac_launch_count.restype = ctypes.c_longlong
     L.ac_free.argtypes = [vp]
@@ -231,6 +245,29 @@ class Context:
         if forcing is not None:
             f = forcing if isinstance(forcing, AcForcing) else AcForcing.from_tuple(forcing)
         _check(self._lib.ac_step(self._ctx, float(dt), ctypes.byref(f) if f is not None else None), "ac_step")
+
+    def ac_substep(self, s, dt, forcing=None):
+        f = None
+        if forcing is not None:
+            f = forcing if isinstance(forcing, AcForcing) else AcForcing.from_tuple(forcing)
+        _check(self._lib.ac_substep(self._ctx, int(s), float(dt), ctypes.byref(f) if f is not None else None),
+               "ac_substep")
+
+    def ac_state_layout(self):
+        info = AcLayoutInfo()
+        _check(self._lib.ac_state_layout(self._ctx, ctypes.byref(info)), "ac_state_layout")
+        return info
+
+    def ac_field_device_ptr(self, q):
+        p = self._lib.ac_field_device_ptr(self._ctx, int(q))
+        if not p:
+            raise AcError("ac_field_device_ptr failed")
+        return int(p)
+
+    def ac_reduce_raw(self):
+        out = (ctypes.c_double * 6)()
+        _check(self._lib.ac_reduce_raw(self._ctx, out), "ac_reduce_raw")
+        return tuple(out)
 
     def ac_reduce(self):
         d = AcDiag()

@@ -299,8 +299,9 @@ void fill_march_coef(const ac_ctx* ctx, ac::MarchCoef<E>& c, double dt, int s, c
     c.rk_b = S::of(RK_BETA[s] * dt);
 }
 
+// substeps [s_begin, s_end) of one RK3 step (ac_step: 0..3; ac_substep: one)
 template <typename T>
-int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
+int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s_begin = 0, int s_end = 3) {
     const ac::Layout& L = ctx->L;
     const ac_grid& g = ctx->grid;
     T* ftab = (T*)(ctx->ws + ctx->cv.ftab_off);
@@ -319,7 +320,7 @@ int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
         a.nz_full = g.nz;
         a.cz = ctx->cz;
         a.has_forcing = forcing ? 1 : 0;
-        for (int s = 0; s < 3; s++) {
+        for (int s = s_begin; s < s_end; s++) {
             a.substep = s;
             fill_march_coef<E>(ctx, a.c, dt, s, forcing);
             for (int q = 0; q < AC_NFIELDS; q++) a.out[q] = (E*)ctx->field_ptr(1 - ctx->cur, q);
@@ -356,7 +357,7 @@ int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
             a.p.fim[i] = forcing ? (T)forcing->im[i] : T(0);
         }
         a.ftab = ftab;
-        for (int s = 0; s < 3; s++) {
+        for (int s = s_begin; s < s_end; s++) {
             a.p.substep = s;
             a.p.rk_a = (s == 0) ? T(0) : (T)(RK_BETA[s] * RK_ALPHA[s] / RK_BETA[s - 1]);
             a.p.rk_b = (T)(RK_BETA[s] * dt);
@@ -673,10 +674,52 @@ int ac_step(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
     return ctx->dtype == AC_F64 ? step_t<double>(ctx, dt, forcing) : step_t<float>(ctx, dt, forcing);
 }
 
+int ac_substep(ac_ctx* ctx, int s, double dt, const ac_forcing* forcing) {
+    if (!ctx || s < 0 || s > 2) return AC_EINVAL;
+    if (!(dt > 0.0) || !std::isfinite(dt)) return AC_EINVAL;
+    if (!ctx->loaded) return AC_ESTATE;
+    return ctx->dtype == AC_F64 ? step_t<double>(ctx, dt, forcing, s, s + 1) : step_t<float>(ctx, dt, forcing, s, s + 1);
+}
+
+int ac_state_layout(const ac_ctx* ctx, ac_layout_info* out) {
+    if (!ctx || !out) return AC_EINVAL;
+    const ac::Layout& L = ctx->L;
+    out->elem_bytes = (int)store_elem_size(ctx->dtype, ctx->packed);
+    out->packed_pairs = ctx->packed ? 1 : 0;
+    out->gx = L.gx;
+    out->pitch = L.pitch;
+    out->my = L.my;
+    out->mz = L.mz;
+    out->plane_elems = L.plane;
+    out->field_elems = L.field;
+    return AC_OK;
+}
+
+void* ac_field_device_ptr(ac_ctx* ctx, int q) {
+    if (!ctx || q < 0 || q >= AC_NFIELDS) return nullptr;
+    return ctx->field_ptr(ctx->cur, q);
+}
+
 int ac_reduce(ac_ctx* ctx, ac_diag* out) {
     if (!ctx || !out) return AC_EINVAL;
     if (!ctx->loaded) return AC_ESTATE;
     return ctx->dtype == AC_F64 ? reduce_t<double>(ctx, out) : reduce_t<float>(ctx, out);
+}
+
+int ac_reduce_raw(ac_ctx* ctx, double out[6]) {
+    if (!ctx || !out) return AC_EINVAL;
+    if (!ctx->loaded) return AC_ESTATE;
+    ac_diag d;
+    const int rc = ctx->dtype == AC_F64 ? reduce_t<double>(ctx, &d) : reduce_t<float>(ctx, &d);
+    if (rc != AC_OK) return rc;
+    const ac::RedVals& r = *ctx->host_result;
+    out[0] = r.su;
+    out[1] = r.mu;
+    out[2] = r.sb;
+    out[3] = r.mb;
+    out[4] = r.lmin;
+    out[5] = r.lmax;
+    return AC_OK;
 }
 
 int ac_forcing_params(double k_f, double helicity, double cs, const ac_grid* grid, double u1, double u2, double u3,
