@@ -85,6 +85,9 @@ def ring_exchange(send_up, send_dn, recv_lo, recv_hi, dist, rank, world):
     import torch
     up, dn = (rank + 1) % world, (rank - 1) % world
     s_up, s_dn = torch.stack(list(send_up)), torch.stack(list(send_dn))
+    if s_up.is_cuda and dist.get_backend() != "nccl":
+        # gloo moves host memory: stage through the CPU (test set-up: several ranks sharing one GPU)
+        s_up, s_dn = s_up.cpu(), s_dn.cpu()
     r_lo, r_hi = torch.empty_like(s_up), torch.empty_like(s_dn)
     ops = [dist.P2POp(dist.isend, s_up, up), dist.P2POp(dist.isend, s_dn, dn),
            dist.P2POp(dist.irecv, r_lo, dn), dist.P2POp(dist.irecv, r_hi, up)]
@@ -141,3 +144,53 @@ class SlabGroupInProcess:
     def free(self):
         for s in self.slabs:
             s.ctx.ac_free()
+
+
+class SlabRank:
+    """One process per rank (torchrun): this rank's slab of the box, exchanged through torch.distributed."""
+
+    def __init__(self, global_shape, lengths, dist, dtype=binding.AC_F64, device="cuda:0", **kw):
+        self.dist, self.rank, self.world = dist, dist.get_rank(), dist.get_world_size()
+        self.shape, self.lengths, self.kw = tuple(global_shape), tuple(lengths), kw
+        self.slab = Slab(global_shape, lengths, self.rank, self.world, dtype, device=device, **kw)
+
+    def forcing_from_draws(self, u1, u2, u3, dt, f0):
+        """Eq. 4-6 for the GLOBAL box (the slab's own context would take its shorter l_z for the box length)."""
+        f = binding.ac_forcing_params(self.kw.get("k_f", 3.0), self.kw.get("helicity", 0.0), self.kw.get("cs", 1.0),
+                                      self.shape, self.lengths, u1, u2, u3, dt, f0)
+        return (tuple(f.k), f.phase, tuple(f.re), tuple(f.im))
+
+    def exchange(self):
+        if self.world == 1:
+            return                                  # the rank's own periodic images are already right
+        self.slab.ctx.synchronize()
+        ring_exchange(*self.slab.halo(), self.dist, self.rank, self.world)
+
+    def load_state(self, state):
+        """state: the GLOBAL (7, nz, ny, nx) array (every rank generates the same seeded input) or this rank's slab."""
+        nzl = self.slab.nzl
+        if state.shape[1] != nzl:
+            state = state[:, self.rank * nzl:(self.rank + 1) * nzl]
+        self.slab.ctx.ac_load_state(np.ascontiguousarray(state))
+        self.exchange()
+
+    def step(self, dt, forcing=None):
+        f = rank_forcing(forcing, self.slab.z0)
+        for sub in range(3):
+            self.slab.ctx.ac_substep(sub, dt, f)
+            self.exchange()
+
+    def reduce(self):
+        import torch
+        raw = torch.tensor(self.slab.ctx.ac_reduce_raw(), dtype=torch.float64)
+        if self.world > 1:
+            allr = [torch.empty_like(raw) for _ in range(self.world)]
+            dev = raw.cuda() if self.dist.get_backend() == "nccl" else raw
+            allr = [torch.empty_like(dev) for _ in range(self.world)]
+            self.dist.all_gather(allr, dev)
+            raws = [tuple(t.cpu().tolist()) for t in allr]
+        else:
+            raws = [tuple(raw.tolist())]
+        nz, ny, nx = self.shape
+        h = min(self.lengths[0] / nx, self.lengths[1] / ny, self.lengths[2] / nz)
+        return combine_raw(raws, nz * ny * nx, h, self.kw.get("nu", 0.0), self.kw.get("eta", 0.0), self.kw.get("cs", 1.0))

@@ -66,3 +66,32 @@ def test_three_substeps_equal_one_step():
         b.ac_substep(3, 1e-3, f)
     a.ac_free()
     b.ac_free()
+
+
+def test_slab_ranks_as_processes(tmp_path):
+    """The multi-process path (slab.SlabRank under torchrun, world_size 2) end to end.  Both ranks share the one GPU
+    and exchange through gloo with host staging; with NCCL on two GPUs only the transport differs."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+           "127.0.0.1", "--master-port", "29551", os.path.join(root, "tests", "slab_worker.py"), str(tmp_path)]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=root)
+    assert r.returncode == 0, r.stderr[-3000:]
+    got = np.concatenate([np.load(tmp_path / ("slab_%d.npy" % k)) for k in range(2)], axis=1)
+    shape = (32, 24, 32)
+    lengths = (2 * math.pi, 1.5 * math.pi, 3.0 * math.pi)
+    one = binding.Context(shape, lengths, binding.AC_F64, nu=5e-3, eta=4e-3, cs=1.0, k_f=3, helicity=1.0)
+    one.ac_load_state(inputs.smooth_strong_state(shape, 41))
+    dt = 2e-3
+    for s in range(2):
+        one.ac_step(dt, one.ac_forcing_from_draws(0.3 + 0.1 * s, 0.6, 0.2, dt, 0.02))
+    err = helpers.max_group_error(got, one.ac_store_state())
+    d = one.ac_reduce()
+    diag = np.load(tmp_path / "diag.npy")
+    one.ac_free()
+    print("2 processes:", err)
+    assert err <= 1e-13
+    for v, key in zip(diag, ("urms", "brms", "umax", "bmax", "dt_cfl")):
+        assert abs(v - d[key]) <= 1e-12 * abs(d[key]), key
