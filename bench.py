@@ -333,6 +333,76 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_slab(args):
+    """N ranks share ONE box as z slabs: strong scaling, halo planes exchanged after every
+    substep through torch.distributed (NCCL).  fp64 only.  Not the default for --gpus N (that is "replicas only")."""
+    import torch
+    import torch.distributed as dist
+    from paper_2012_08758_b200 import binding, inputs, slab
+
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    else:
+        dist.init_process_group("gloo", init_method="tcp://127.0.0.1:29561", rank=0, world_size=1)
+    rank = dist.get_rank()
+    n = args.n
+    cfg = workload(n)
+    nu = cfg["nu"]
+    rk = slab.SlabRank((n, n, n), TWO_PI3, dist, binding.AC_F64, device="cuda:%d" % local_rank, nu=nu, eta=nu, cs=1.0,
+                       k_f=3.0, helicity=cfg["sigma"])
+    nzl = rk.slab.nzl
+    local = np.empty((7, nzl, n, n))
+    for q, field in enumerate(inputs.solenoidal_state_fields(n, cfg["seed"])):
+        local[q] = field[rank * nzl:(rank + 1) * nzl]
+    del field
+    rk.load_state(local)
+    dt = rk.reduce()["dt_cfl"]
+    draws = [inputs.counter_uniforms(cfg["seed"] + 7, s) for s in range(args.warmup + args.steps)]
+    forcings = [rk.forcing_from_draws(*u, dt, 0.02) for u in draws]
+    for s in range(args.warmup):
+        rk.step(dt, forcings[s])
+    torch.cuda.synchronize()
+    dist.barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = rk.slab.ctx.ac_launch_count()
+    e0.record(rk.slab.ctx.stream)
+    for s in range(args.steps):
+        rk.step(dt, forcings[args.warmup + s])
+    e1.record(rk.slab.ctx.stream)
+    torch.cuda.synchronize()
+    dist.barrier()
+    clocks = sampler.stop()
+    total_ms = max_over_ranks(e0.elapsed_time(e1), dist if world > 1 else None, "cuda")
+    launches = rk.slab.ctx.ac_launch_count() - l0
+    diag = rk.reduce()
+    ms_per_step = total_ms / args.steps
+    value = n ** 3 / (ms_per_step * 1e-3)
+    peak, peak_src = measured_peak()
+    alg = WORDS_PER_CELL_STEP / 3.0 * 8 * n ** 3 / world        # per rank and launch
+    achieved = alg / (ms_per_step / 3.0 * 1e-3) / 1e9
+    halo_bytes = 2 * 7 * 3 * rk.slab.info.plane_elems * 8
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "grid": [n, n, n], "nu": nu, "eta": nu, "helicity": cfg["sigma"], "k_f": 3,
+                       "f0": 0.02, "dt": dt, "parallelism": "z slabs x%d, halo exchange per substep" % world,
+                       "l2": "state far larger than L2; no flush needed",
+                       "halo_bytes_per_rank_per_substep": halo_bytes},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": committed_traffic("f64"), "peak_source": peak_src,
+                         "kernel": "substep (per rank; halo exchange and ghost kernels charged to it)"},
+            "cpu_baseline": None, "e2e": None, "gpu_launches": launches, "clocks": clocks,
+            "diag": {k: diag[k] for k in ("urms", "brms")}}))
+    dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -346,11 +416,15 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-sample", type=int, default=128, help="box size of the bounded oracle sample")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--slab", action="store_true",
+                    help="N ranks share one box as z slabs with a halo exchange per substep (strong scaling, fp64)")
     ap.add_argument("--paper-protocol", action="store_true",
                     help="the paper's benchmark set-up (PAPER.md:533): all fields U[0,1), no forcing, dt = 1.19209e-7")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.slab:
+        run_slab(args)
     else:
         run_ours(args)
 
