@@ -20,6 +20,7 @@
 #include "mhd_cell.cuh"
 #include "reduce_tma.cuh"
 #include "substep_march.cuh"
+#include "substep_pair.cuh"
 #include "vec2.cuh"
 
 namespace {
@@ -143,7 +144,7 @@ struct ac_ctx {
     double c_u, c_nu;
     int upwind;          // 1 = upwinded continuity equation (G17); default 0
     int mixed;           // 0 = bidiagonal mixed stencil (G2, default), 1 = tensor product (direct kernel only)
-    int variant;         // requested: 0 = scatter-march, 1 = direct
+    int variant;         // requested: 0 = pair-march (default), 1 = direct, 2 = scatter-march (one cell per thread)
     bool march;          // the kernel actually used (fp32 with odd nz falls back to direct)
     bool packed;         // fp32 cells stored as (z, z + nz/2) pairs
     ac::Layout L;        // layout in storage elements
@@ -320,11 +321,24 @@ int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s_begin = 0, i
         a.nz_full = g.nz;
         a.cz = ctx->cz;
         a.has_forcing = forcing ? 1 : 0;
+        a.wrap_z = 1;
         for (int s = s_begin; s < s_end; s++) {
             a.substep = s;
             fill_march_coef<E>(ctx, a.c, dt, s, forcing);
             for (int q = 0; q < AC_NFIELDS; q++) a.out[q] = (E*)ctx->field_ptr(1 - ctx->cur, q);
             dim3 grd((L.nx + ac::M_TX - 1) / ac::M_TX, (L.ny + ac::M_TY - 1) / ac::M_TY, ctx->nchunks);
+            if (ctx->variant == 0) {
+                // pair-march: one launch does the substep and the ghost zones of the buffer it writes
+                if (ctx->upwind)
+                    ac::substep_pair_kernel<T, true><<<grd, ac::M_THREADS, ac::P_SMEM_BYTES, ctx->stream>>>(
+                        a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
+                else
+                    ac::substep_pair_kernel<T, false><<<grd, ac::M_THREADS, ac::P_SMEM_BYTES, ctx->stream>>>(
+                        a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
+                ctx->launches++;
+                ctx->cur = 1 - ctx->cur;
+                continue;
+            }
             if (ctx->upwind)
                 ac::substep_march_kernel<T, true><<<grd, ac::M_THREADS, ac::M_SMEM_BYTES, ctx->stream>>>(
                     a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
@@ -489,7 +503,7 @@ namespace {
 // choose the kernel and the device layout for the context's variant; builds the TMA maps
 int configure(ac_ctx* ctx) {
     const ac_grid* g = &ctx->grid;
-    ctx->march = ctx->variant == 0 && ctx->mixed == 0 && (ctx->dtype == AC_F64 || can_pack(g));
+    ctx->march = ctx->variant != 1 && ctx->mixed == 0 && (ctx->dtype == AC_F64 || can_pack(g));
     ctx->packed = ctx->march && ctx->dtype == AC_F32;
     ctx->L = layout_for(g, ctx->dtype, ctx->packed);
     ctx->cv = carve(ctx->L, store_elem_size(ctx->dtype, ctx->packed), elem_size(ctx->dtype), g->nz);
@@ -504,12 +518,18 @@ int configure(ac_ctx* ctx) {
         if (rc == AC_OK) rc = make_state_map(&ctx->map_p[b], ctx->field_ptr(b, 0), ctx->L, ac::M_TX, ac::M_TY, 4);
         if (rc != AC_OK) return rc;
     }
-    const void* kernels[4] = {(const void*)ac::substep_march_kernel<double, false>,
+    const void* kernels[8] = {(const void*)ac::substep_march_kernel<double, false>,
                               (const void*)ac::substep_march_kernel<double, true>,
                               (const void*)ac::substep_march_kernel<float, false>,
-                              (const void*)ac::substep_march_kernel<float, true>};
-    for (int k = (ctx->dtype == AC_F64 ? 0 : 2), e = k + 2; k < e; k++) {
-        cudaError_t ea = cudaFuncSetAttribute(kernels[k], cudaFuncAttributeMaxDynamicSharedMemorySize, ac::M_SMEM_BYTES);
+                              (const void*)ac::substep_march_kernel<float, true>,
+                              (const void*)ac::substep_pair_kernel<double, false>,
+                              (const void*)ac::substep_pair_kernel<double, true>,
+                              (const void*)ac::substep_pair_kernel<float, false>,
+                              (const void*)ac::substep_pair_kernel<float, true>};
+    for (int k = 0; k < 8; k++) {
+        if ((ctx->dtype == AC_F64) != (k % 4 < 2)) continue;
+        cudaError_t ea = cudaFuncSetAttribute(kernels[k], cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              k < 4 ? ac::M_SMEM_BYTES : ac::P_SMEM_BYTES);
         if (ea != cudaSuccess) return cuda_fail(ea, "cudaFuncSetAttribute(march kernel smem)");
     }
     // z chunks: every chunk re-reads 6 planes, every wave of CTAs costs (planes + 6) iterations;
@@ -823,7 +843,7 @@ int ac_set_mixed(ac_ctx* ctx, int mode) {
 
 int ac_set_variant(ac_ctx* ctx, int variant) {
     if (!ctx) return AC_EINVAL;
-    if (variant != 0 && variant != 1) return AC_EINVAL;
+    if (variant < 0 || variant > 2) return AC_EINVAL;
     if (variant == ctx->variant) return AC_OK;
     // the variants use different device layouts in fp32: a loaded state would have to be re-packed
     cudaStreamSynchronize(ctx->stream);

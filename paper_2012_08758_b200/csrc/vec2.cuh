@@ -115,6 +115,14 @@ __device__ __forceinline__ f2 vswap(f2 a) {
     return vmake(hi, lo);
 }
 
+// load through L2 only (data another thread of the CTA has just stored)
+__device__ __forceinline__ double vldcg(const double* p) { return __ldcg(p); }
+__device__ __forceinline__ f2 vldcg(const f2* p) {
+    f2 r;
+    r.v = __ldcg(reinterpret_cast<const unsigned long long*>(p));
+    return r;
+}
+
 template <typename E>
 __device__ __forceinline__ E vzero() {
     return Splat<E>::of(0.0);

@@ -13,7 +13,7 @@ from helpers import TWO_PI3
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = [0, 1]
+VARIANTS = [0, 1, 2]          # 0 = pair-march (default), 1 = direct, 2 = scatter-march with a ghost-zone kernel
 
 
 def make_ctx(shape, dtype=binding.AC_F64, lengths=TWO_PI3, variant=0, **kw):
@@ -173,7 +173,8 @@ def test_variants_agree_and_run_to_run_determinism():
         res.append((ctx.ac_store_state(), ctx.ac_reduce()))
         ctx.ac_free()
     assert np.array_equal(res[0][0], res[-1][0]) and res[0][1] == res[-1][1]       # same variant twice: bitwise
-    assert helpers.max_group_error(res[1][0], res[0][0]) <= 1e-13
+    for other in res[1:-1]:
+        assert helpers.max_group_error(other[0], res[0][0]) <= 1e-13
 
 
 def test_state_errors_and_device_buffers():
@@ -197,9 +198,9 @@ def test_state_errors_and_device_buffers():
     assert torch.equal(out, dev)
     n0 = ctx.ac_launch_count()
     ctx.ac_step(1e-3, None)
-    assert ctx.ac_launch_count() - n0 == 6            # three fused substep kernels, each followed by the ghost-zone kernel
+    assert ctx.ac_launch_count() - n0 == 3            # three fused substep kernels (ghost zones included), nothing else
     ctx.ac_step(1e-3, ctx.ac_make_forcing(1, 0, 1e-3, 0.02))
-    assert ctx.ac_launch_count() - n0 == 13           # + forcing table kernel
+    assert ctx.ac_launch_count() - n0 == 7            # + forcing table kernel
     # a NaN in the state is reported
     bad = state.copy()
     bad[5, 3, 3, 3] = np.nan
