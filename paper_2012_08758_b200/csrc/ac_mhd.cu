@@ -161,6 +161,8 @@ struct ac_ctx {
     CUtensorMap map_prev[2];   // and interior-tile boxes (previous state of the 2N update)
     CUtensorMap map_a[2];      // tile + halo boxes of the three A fields (reductions)
     CUtensorMap map_p[2];      // interior-tile boxes of ln rho and u (reductions)
+    CUtensorMap map_qin[2];    // pair-march kernel: 16 x 16 tile + halo boxes
+    CUtensorMap map_qprev[2];  // and interior-tile boxes
     int cz, nchunks;           // z chunking of the march kernel
 
     void* field_ptr(int buf, int q) const { return ws + ((size_t)buf * AC_NFIELDS + q) * cv.field_bytes; }
@@ -287,6 +289,9 @@ void fill_march_coef(const ac_ctx* ctx, ac::MarchCoef<E>& c, double dt, int s, c
     c.nc20yz = S::of(-(c20[1] + c20[2]));
     c.nc20xz = S::of(-(c20[0] + c20[2]));
     c.nc20xy = S::of(-(c20[0] + c20[1]));
+    c.c20x = S::of(c20[0]);
+    c.c20y = S::of(c20[1]);
+    c.c20z = S::of(c20[2]);
     c.nu = S::of(ctx->nu);
     c.eta = S::of(ctx->eta);
     c.ncs2 = S::of(-(ctx->cs * ctx->cs));
@@ -328,23 +333,21 @@ int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s_begin = 0, i
             for (int q = 0; q < AC_NFIELDS; q++) a.out[q] = (E*)ctx->field_ptr(1 - ctx->cur, q);
             dim3 grd((L.nx + ac::M_TX - 1) / ac::M_TX, (L.ny + ac::M_TY - 1) / ac::M_TY, ctx->nchunks);
             if (ctx->variant == 0) {
-                // pair-march: one launch does the substep and the ghost zones of the buffer it writes
+                // pair-march: 16 x 16 tiles, a thread owns two cells
+                dim3 gq((L.nx + ac::Q_TX - 1) / ac::Q_TX, (L.ny + ac::Q_TY - 1) / ac::Q_TY, ctx->nchunks);
                 if (ctx->upwind)
-                    ac::substep_pair_kernel<T, true><<<grd, ac::M_THREADS, ac::P_SMEM_BYTES, ctx->stream>>>(
-                        a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
+                    ac::substep_pair_kernel<T, true><<<gq, ac::Q_THREADS, ac::Q_SMEM_BYTES, ctx->stream>>>(
+                        a, ctx->map_qin[ctx->cur], ctx->map_qprev[1 - ctx->cur]);
                 else
-                    ac::substep_pair_kernel<T, false><<<grd, ac::M_THREADS, ac::P_SMEM_BYTES, ctx->stream>>>(
-                        a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
-                ctx->launches++;
-                ctx->cur = 1 - ctx->cur;
-                continue;
-            }
-            if (ctx->upwind)
+                    ac::substep_pair_kernel<T, false><<<gq, ac::Q_THREADS, ac::Q_SMEM_BYTES, ctx->stream>>>(
+                        a, ctx->map_qin[ctx->cur], ctx->map_qprev[1 - ctx->cur]);
+            } else if (ctx->upwind) {
                 ac::substep_march_kernel<T, true><<<grd, ac::M_THREADS, ac::M_SMEM_BYTES, ctx->stream>>>(
                     a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
-            else
+            } else {
                 ac::substep_march_kernel<T, false><<<grd, ac::M_THREADS, ac::M_SMEM_BYTES, ctx->stream>>>(
                     a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
+            }
             ctx->launches++;
             // S1: refresh the ghost zones of the buffer just written
             const int nb_rows = 2 * ac::R * L.my + 2 * ac::R * L.nz;
@@ -516,6 +519,8 @@ int configure(ac_ctx* ctx) {
         if (rc == AC_OK) rc = make_state_map(&ctx->map_prev[b], ctx->field_ptr(b, 0), ctx->L, ac::M_TX, ac::M_TY);
         if (rc == AC_OK) rc = make_state_map(&ctx->map_a[b], ctx->field_ptr(b, ac::AX), ctx->L, ac::M_WX, ac::M_WY, 3);
         if (rc == AC_OK) rc = make_state_map(&ctx->map_p[b], ctx->field_ptr(b, 0), ctx->L, ac::M_TX, ac::M_TY, 4);
+        if (rc == AC_OK) rc = make_state_map(&ctx->map_qin[b], ctx->field_ptr(b, 0), ctx->L, ac::Q_WX, ac::Q_WY);
+        if (rc == AC_OK) rc = make_state_map(&ctx->map_qprev[b], ctx->field_ptr(b, 0), ctx->L, ac::Q_TX, ac::Q_TY);
         if (rc != AC_OK) return rc;
     }
     const void* kernels[8] = {(const void*)ac::substep_march_kernel<double, false>,
@@ -529,13 +534,14 @@ int configure(ac_ctx* ctx) {
     for (int k = 0; k < 8; k++) {
         if ((ctx->dtype == AC_F64) != (k % 4 < 2)) continue;
         cudaError_t ea = cudaFuncSetAttribute(kernels[k], cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                              k < 4 ? ac::M_SMEM_BYTES : ac::P_SMEM_BYTES);
+                                              k < 4 ? ac::M_SMEM_BYTES : ac::Q_SMEM_BYTES);
         if (ea != cudaSuccess) return cuda_fail(ea, "cudaFuncSetAttribute(march kernel smem)");
     }
     // z chunks: every chunk re-reads 6 planes, every wave of CTAs costs (planes + 6) iterations;
     // pick the chunk count that minimises waves x (planes per chunk + 6)
     const int nzp = ctx->L.nz;
-    const long tiles = (long)((ctx->L.nx + ac::M_TX - 1) / ac::M_TX) * ((ctx->L.ny + ac::M_TY - 1) / ac::M_TY);
+    const int tile_x = ctx->variant == 0 ? ac::Q_TX : ac::M_TX, tile_y = ctx->variant == 0 ? ac::Q_TY : ac::M_TY;
+    const long tiles = (long)((ctx->L.nx + tile_x - 1) / tile_x) * ((ctx->L.ny + tile_y - 1) / tile_y);
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
     long best_cost = -1;

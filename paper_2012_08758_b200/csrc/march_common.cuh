@@ -47,7 +47,7 @@ struct MarchCoef {
     E cm3xy[3], cm3xz[3], ncm3xz[3], cm3yz[3], ncm3yz[3];
     // A role
     E c2x[3], c2y[3], c2z[3], nc2x[3], nc2y[3], nc2z[3];
-    E c20all, nc20yz, nc20xz, nc20xy;
+    E c20all, nc20yz, nc20xz, nc20xy, c20x, c20y, c20z;
     E cmxy[3], cmxz[3], ncmxz[3], cmyz[3], ncmyz[3];
     // upwind correction of the continuity equation (G17; UPW kernels only): delta6 / (60 h)
     E c6x[3], c6y[3], c6z[3], c60x, c60y, c60z;
