@@ -102,30 +102,24 @@ __device__ __forceinline__ void q_join(double& a, uint32_t lo, uint32_t hi) { a 
 __device__ __forceinline__ void q_join(f2& a, uint32_t lo, uint32_t hi) { a.v = ((unsigned long long)hi << 32) | lo; }
 
 template <typename E>
-__device__ __forceinline__ void q_st4(uint32_t taddr, E a, E b, E c, E d) {
-    uint32_t r[8];
-    q_split(a, r[0], r[1]);
-    q_split(b, r[2], r[3]);
-    q_split(c, r[4], r[5]);
-    q_split(d, r[6], r[7]);
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(r[0]),
-                 "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
-                 : "memory");
-}
-template <typename E>
-__device__ __forceinline__ void q_st2(uint32_t taddr, E a, E b) {
-    uint32_t r[4];
-    q_split(a, r[0], r[1]);
-    q_split(b, r[2], r[3]);
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(r[0]), "r"(r[1]),
-                 "r"(r[2]), "r"(r[3])
-                 : "memory");
-}
-template <typename E>
 __device__ __forceinline__ void q_st1(uint32_t taddr, E a) {
     uint32_t r[2];
     q_split(a, r[0], r[1]);
     asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(r[0]), "r"(r[1]) : "memory");
+}
+// wider stores as single-element stores: a tcgen05.st.x8 wants its 8 source registers consecutive, which cost 8 moves
+// per store in the loop; x2 stores take each 8-byte value where it was computed
+template <typename E>
+__device__ __forceinline__ void q_st2(uint32_t taddr, E a, E b) {
+    q_st1<E>(taddr, a);
+    q_st1<E>(taddr + 2, b);
+}
+template <typename E>
+__device__ __forceinline__ void q_st4(uint32_t taddr, E a, E b, E c, E d) {
+    q_st1<E>(taddr, a);
+    q_st1<E>(taddr + 2, b);
+    q_st1<E>(taddr + 4, c);
+    q_st1<E>(taddr + 6, d);
 }
 // loads return raw registers; they hold the data only after q_wait_ld + q_tie (the tie takes them as in-out
 // operands of an ordered asm so that no use can be scheduled above the wait)
@@ -311,7 +305,9 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
     const Layout& L = a.L;
     const MarchCoef<E>& c = a.c;
     const int tid = threadIdx.x;
-    const int warp = tid >> 5, lane = tid & 31;
+    // the shuffles tell the compiler that the warp index (and what derives from it: role, tensor-memory addresses)
+    // is warp-uniform, so that it lives in uniform registers
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0), lane = tid & 31;
     // warps 0-3 = U  4-7 = A  8 = producer (lane 0)  9 = owns the tensor memory  10, 11 idle
     const int wp = warp & 3;                   // U warp w and A warp w + 4 share tensor-memory lanes and column pairs
     const int tx = lane & 15;
@@ -351,7 +347,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
     q_fence_before();
     __syncthreads();
     q_fence_after();
-    const uint32_t tm = *tmem_word + ((uint32_t)(wp * 32) << 16);
+    const uint32_t tm = __shfl_sync(0xffffffffu, *tmem_word, 0) + ((uint32_t)(wp * 32) << 16);
 
     const int cell_off = (ty0 + R) * Q_WX + tx + Q_HX;
 
