@@ -141,6 +141,15 @@ def diagnostics(state, lengths, bext=(0.0, 0.0, 0.0)):
             "lnrho_min": out[4], "lnrho_max": out[5], "nonfinite": int(out[6])}
 
 
+def diagnostics_ext(state, lengths, bext=(0.0, 0.0, 0.0), mixed="bidiagonal"):
+    """<omega.u>, <j.B> (Eq. 11) and the largest Alfven speed (G15): orc_diag_ext."""
+    state = np.ascontiguousarray(state, dtype=np.float64)
+    p = make_params(state.shape[1:], lengths, bext=bext, mixed=mixed)
+    out = np.zeros(3)
+    lib().orc_diag_ext(_ptr(state), ctypes.byref(p), _ptr(out))
+    return {"kin_hel": out[0], "cur_hel": out[1], "va_max": out[2]}
+
+
 def der1_field(f, a, lengths):
     f = np.ascontiguousarray(f, dtype=np.float64)
     p = make_params(f.shape, lengths)

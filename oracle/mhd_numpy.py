@@ -228,6 +228,37 @@ def diagnostics(state, lengths, bext=(0.0, 0.0, 0.0)):
     }
 
 
+def diagnostics_ext(state, lengths, bext=(0.0, 0.0, 0.0), mixed="bidiagonal"):
+    """<omega.u>, <j.B> (Eq. 11; mu0 = rho0 = 1) and max |B| / sqrt(rho) (the Alfven term of G15)."""
+    h = grid_spacing(state.shape[1:], lengths)
+    u = [state[UX], state[UY], state[UZ]]
+    a = [state[AX], state[AY], state[AZ]]
+    om = [der1(u[2], 1, h) - der1(u[1], 2, h), der1(u[0], 2, h) - der1(u[2], 0, h), der1(u[1], 0, h) - der1(u[0], 1, h)]
+    B = curl_a(state, h)
+    B = [B[i] + bext[i] for i in range(3)]
+    jj = []
+    for i in range(3):
+        gd = der2(a[i], i, h)
+        for j in range(3):
+            if j != i:
+                gd = gd + dermix(a[j], min(i, j), max(i, j), h, mixed)
+        jj.append(gd - (der2(a[i], 0, h) + der2(a[i], 1, h) + der2(a[i], 2, h)))
+    hk = sum(om[i] * u[i] for i in range(3)).mean()
+    hc = sum(jj[i] * B[i] for i in range(3)).mean()
+    va2 = (sum(B[i] ** 2 for i in range(3)) * np.exp(-state[LNRHO])).max()
+    return {"kin_hel": float(hk), "cur_hel": float(hc), "va_max": float(np.sqrt(va2))}
+
+
+def cfl_dt_alfven(umax, va_max, shape, lengths, nu, eta, cs, c_u=0.4, c_nu=0.25):
+    """The optional Alfven-speed form of G15: the signal speed c_s becomes sqrt(c_s^2 + max v_A^2)."""
+    h = min(grid_spacing(shape, lengths))
+    dt_adv = c_u * h / (umax + np.sqrt(cs * cs + va_max * va_max))
+    d = max(nu, eta)
+    if d <= 0.0:
+        return dt_adv
+    return min(dt_adv, c_nu * h * h / d)
+
+
 def cfl_dt(umax, shape, lengths, nu, eta, cs, c_u=0.4, c_nu=0.25):
     """dt = min(C_u h/(max|u| + c_s), C_nu h^2/max(nu, eta)), h = min spacing (reading G15;
     parity unpinned by the paper: the paper's benchmark uses a constant time step)."""

@@ -271,6 +271,43 @@ void orc_diag(const double* state, const orc_params* p, double out[7]) {
     out[6] = (double)bad;
 }
 
+/* Extended diagnostics (NEXT-4): volume means of the kinetic helicity omega.u, omega = curl u, and of the current
+ * helicity j.B (Eq. 11; mu0 = rho0 = 1; j = grad div A - lap A as in Eq. 2, reading G4;
+ * B includes the external field), and the largest Alfven speed |B| / sqrt(rho) (the optional term of the CFL rule,
+ * reading G15).  In a periodic box <j> = 0, so the mean of j.B equals that of the fluctuating parts j'.b' of Eq. 11.
+ * out: <omega.u>, <j.B>, max |B| rho^(-1/2) */
+void orc_diag_ext(const double* state, const orc_params* p, double out[3]) {
+    const size_t n = (size_t)p->nx * p->ny * p->nz;
+    const double* lnrho = state;
+    const double* u[3] = {state + n, state + 2 * n, state + 3 * n};
+    const double* A[3] = {state + 4 * n, state + 5 * n, state + 6 * n};
+    double hk = 0.0, hc = 0.0, va2 = 0.0;
+    for (long z = 0; z < p->nz; z++)
+        for (long y = 0; y < p->ny; y++)
+            for (long x = 0; x < p->nx; x++) {
+                const size_t c = (size_t)x + (size_t)p->nx * ((size_t)y + (size_t)p->ny * (size_t)z);
+                double om[3], B[3], jj[3];
+                om[0] = der1(u[2], p, x, y, z, 1) - der1(u[1], p, x, y, z, 2);
+                om[1] = der1(u[0], p, x, y, z, 2) - der1(u[2], p, x, y, z, 0);
+                om[2] = der1(u[1], p, x, y, z, 0) - der1(u[0], p, x, y, z, 1);
+                curl_a(A, p, x, y, z, B);
+                for (int i = 0; i < 3; i++) {
+                    double lap = der2(A[i], p, x, y, z, 0) + der2(A[i], p, x, y, z, 1) + der2(A[i], p, x, y, z, 2);
+                    double s = der2(A[i], p, x, y, z, i);
+                    for (int j = 0; j < 3; j++)
+                        if (j != i) s += dermix(A[j], p, x, y, z, i, j);
+                    jj[i] = s - lap;
+                }
+                hk += om[0] * u[0][c] + om[1] * u[1][c] + om[2] * u[2][c];
+                hc += jj[0] * B[0] + jj[1] * B[1] + jj[2] * B[2];
+                double v2 = (B[0] * B[0] + B[1] * B[1] + B[2] * B[2]) * exp(-lnrho[c]);
+                if (v2 > va2) va2 = v2;
+            }
+    out[0] = hk / (double)n;
+    out[1] = hc / (double)n;
+    out[2] = sqrt(va2);
+}
+
 /* single derivative operators on a whole scalar field, for the operator pins (P1-P3) */
 void orc_der1_field(const double* f, double* out, const orc_params* p, int a) {
     for (long z = 0; z < p->nz; z++)
