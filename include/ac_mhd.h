@@ -50,7 +50,7 @@ typedef enum {
     AC_EINVAL = -1, /* NULL pointer, bad grid (n < 8, nx % 4 != 0), non-positive L or cs, negative nu/eta, bad dt */
     AC_ENOMEM = -2, /* device or host allocation failed / workspace too small */
     AC_ECUDA = -3,  /* CUDA error (sticky); text from ac_strerror(AC_ECUDA) on the same thread */
-    AC_ESTATE = -4  /* ac_step / ac_reduce / ac_store_state before ac_load_state */
+    AC_ESTATE = -4  /* ac_step / ac_reduce / ac_store_state before ac_load_state; a call that is not allowed between substeps */
 } ac_status;
 
 /* Periodic box: n cells and side length per axis; spacing h_a = l_a / n_a (l = 2 pi). */
@@ -132,6 +132,10 @@ int ac_step(ac_ctx* ctx, double dt, const ac_forcing* forcing);
  * pack kernel.  The forcing phase of a rank is the global phase + k_z * z0 with z0 the position of its first plane.
  * Only layouts with packed_pairs == 0 can be exchanged this way (fp64, or fp32 with ac_set_variant(ctx, 1)).
  * ac_substep: substep s = 0, 1, 2 of the 2N-RK3 step; three calls with the same dt and forcing equal ac_step.
+ *   The substeps must come in order (AC_ESTATE otherwise; ac_load_state restarts at 0): between substeps the idle
+ *   state buffer holds the previous state, from which the 2N register is rebuilt.  Therefore, after substep 0 or 1,
+ *   ac_step, ac_load_field, ac_reduce_ext and the HOST-destination forms of ac_store_state / ac_store_field (which
+ *   stage in that buffer) return AC_ESTATE; device-destination stores and ac_reduce stay available.
  * ac_reduce_raw: the unnormalised reductions of this rank's cells, out = {sum |u|^2, max |u|^2, sum |B|^2, max |B|^2,
  * min ln rho, max ln rho}, to be combined across ranks (sum, max, sum, max, min, max).  Synchronises the stream. */
 typedef struct {
@@ -149,6 +153,22 @@ int ac_reduce_raw(ac_ctx* ctx, double out[6]);
  * time step dt = min(C_u h/(umax + cs), C_nu h^2/max(nu, eta)) (G15).  Deterministic (fixed
  * two-stage tree, no floating-point atomics).  Synchronises the stream. */
 int ac_reduce(ac_ctx* ctx, ac_diag* out);
+
+/* Extended diagnostics: volume means of the kinetic helicity omega.u (omega = curl u) and of the
+ * current helicity j.B (Eq. 11, with mu0 = rho0 = 1; j = grad div A - lap A as in
+ * Eq. 2, B = curl A + external field; in a periodic box <j> = 0, so <j.B> is also the mean of the fluctuating parts
+ * j'.b' of Eq. 11), the largest Alfven speed |B| / sqrt(rho), and the CFL step with the Alfven term of reading G15,
+ * dt = min(C_u h / (umax + sqrt(cs^2 + va_max^2)), C_nu h^2 / max(nu, eta)).  Runs ac_reduce plus one gather
+ * kernel; deterministic; synchronises the stream.  Scratch lives in the idle state buffer, so inside a step driven
+ * by ac_substep (after substep 0 or 1) the call returns AC_ESTATE.
+ * ac_reduce_ext_raw: this rank's {sum omega.u, sum j.B, max |B|^2 / rho} for a slab decomposition (sum, sum, max). */
+typedef struct {
+    double kin_hel, cur_hel, va_max;
+    double dt_cfl_alfven;
+    int nonfinite;
+} ac_diag_ext;
+int ac_reduce_ext(ac_ctx* ctx, ac_diag_ext* out);
+int ac_reduce_ext_raw(ac_ctx* ctx, double out[3]);
 
 /* Host helpers for Eq. 4-6 (no device work).
  * ac_forcing_from_draws: u1, u2, u3 in [0, 1) choose the shell vector (index floor(u1*len) into

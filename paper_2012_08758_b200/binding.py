@@ -19,6 +19,7 @@ EXPORTS = (
     "ac_reduce",
     "ac_forcing_from_draws", "ac_forcing_params", "ac_make_forcing", "ac_set_bext", "ac_set_cfl", "ac_set_variant",
     "ac_set_upwind", "ac_set_mixed", "ac_substep", "ac_state_layout", "ac_field_device_ptr", "ac_reduce_raw",
+    "ac_reduce_ext", "ac_reduce_ext_raw",
     "ac_launch_count", "ac_free", "ac_strerror", "ac_version",
 )
 
@@ -56,6 +57,14 @@ class AcDiag(ctypes.Structure):
     _fields_ = [("urms", ctypes.c_double), ("umax", ctypes.c_double), ("brms", ctypes.c_double),
                 ("bmax", ctypes.c_double), ("lnrho_min", ctypes.c_double), ("lnrho_max", ctypes.c_double),
                 ("dt_cfl", ctypes.c_double), ("nonfinite", ctypes.c_int)]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+class AcDiagExt(ctypes.Structure):
+    _fields_ = [("kin_hel", ctypes.c_double), ("cur_hel", ctypes.c_double), ("va_max", ctypes.c_double),
+                ("dt_cfl_alfven", ctypes.c_double), ("nonfinite", ctypes.c_int)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -106,6 +115,10 @@ def load_library():
     L.ac_field_device_ptr.restype = ctypes.c_void_p
     L.ac_reduce_raw.argtypes = [vp, ctypes.POINTER(dbl)]
     L.ac_reduce_raw.restype = i32
+    L.ac_reduce_ext.argtypes = [vp, ctypes.POINTER(AcDiagExt)]
+    L.ac_reduce_ext.restype = i32
+    L.ac_reduce_ext_raw.argtypes = [vp, ctypes.POINTER(dbl)]
+    L.ac_reduce_ext_raw.restype = i32
     L.ac_launch_count.argtypes = [vp]
     L.ac_launch_count.restype = ctypes.c_longlong
     L.ac_free.argtypes = [vp]
@@ -174,8 +187,10 @@ class Context:
         base = self.workspace.data_ptr()
         aligned = (base + 255) // 256 * 256
         self._ctx = ctypes.c_void_p()
-        rc = L.ac_init(ctypes.byref(self._ctx), ctypes.byref(g), self.dtype, float(nu), float(eta), float(cs),
-                       float(k_f), float(helicity), ctypes.c_void_p(aligned), ctypes.c_void_p(self.stream.cuda_stream))
+        with torch.cuda.device(self.device):       # the library records the current device as the context's
+            rc = L.ac_init(ctypes.byref(self._ctx), ctypes.byref(g), self.dtype, float(nu), float(eta), float(cs),
+                           float(k_f), float(helicity), ctypes.c_void_p(aligned),
+                           ctypes.c_void_p(self.stream.cuda_stream))
         _check(rc, "ac_init")
         self._lib = L
 
@@ -273,6 +288,16 @@ class Context:
         d = AcDiag()
         _check(self._lib.ac_reduce(self._ctx, ctypes.byref(d)), "ac_reduce")
         return d.as_dict()
+
+    def ac_reduce_ext(self):
+        d = AcDiagExt()
+        _check(self._lib.ac_reduce_ext(self._ctx, ctypes.byref(d)), "ac_reduce_ext")
+        return d.as_dict()
+
+    def ac_reduce_ext_raw(self):
+        out = (ctypes.c_double * 3)()
+        _check(self._lib.ac_reduce_ext_raw(self._ctx, out), "ac_reduce_ext_raw")
+        return tuple(out)
 
     def ac_forcing_from_draws(self, u1, u2, u3, dt, f0):
         f = AcForcing()

@@ -15,6 +15,7 @@
 #include <type_traits>
 #include <vector>
 
+#include "diag_ext.cuh"
 #include "kernels.cuh"
 #include "layout.cuh"
 #include "mhd_cell.cuh"
@@ -49,7 +50,7 @@ const double W6[3] = {15.0 / 60.0, -6.0 / 60.0, 1.0 / 60.0};
 const double RK_ALPHA[3] = {0.0, -5.0 / 9.0, -153.0 / 128.0};
 const double RK_BETA[3] = {1.0 / 3.0, 15.0 / 16.0, 8.0 / 15.0};
 
-const int RED_BLOCKS = 148 * 8;
+const int RED_BLOCKS = 148 * 8;   // capacity of the partial-result scratch (stage-1 grids are sized from the device's SM count, capped here)
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -164,11 +165,25 @@ struct ac_ctx {
     CUtensorMap map_qin[2];    // pair-march kernel: 16 x 16 tile + halo boxes
     CUtensorMap map_qprev[2];  // and interior-tile boxes
     int cz, nchunks;           // z chunking of the march kernel
+    int device, sms;           // CUDA device ordinal of the context and its SM count
+    int next_substep;          // 0 between full steps; 1, 2 inside a step driven by ac_substep (the idle buffer is live then)
 
     void* field_ptr(int buf, int q) const { return ws + ((size_t)buf * AC_NFIELDS + q) * cv.field_bytes; }
 };
 
 namespace {
+
+// makes the context's device current for the duration of a call (a context may be used while another device is current)
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const ac_ctx* ctx) {
+        if (ctx && cudaGetDevice(&prev) == cudaSuccess && prev != ctx->device) switched = cudaSetDevice(ctx->device) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+};
 
 template <typename T>
 void fill_coeffs(const ac_ctx* ctx, ac::Coeffs<T>& c) {
@@ -411,17 +426,11 @@ int reduce_t(ac_ctx* ctx, ac_diag* out) {
         // 8-byte-element layouts (fp64, packed fp32): TMA plane ring (reduce_tma.cuh)
         const int tiles_x = (L.nx + ac::M_TX - 1) / ac::M_TX, tiles_y = (L.ny + ac::M_TY - 1) / ac::M_TY;
         const int nchunks = (L.nz + ac::RQ_CZ - 1) / ac::RQ_CZ;
-        int sms = 148;
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
-        blocks = (int)std::min<long>((long)tiles_x * tiles_y * nchunks, std::min(3 * sms, RED_BLOCKS));
+        blocks = (int)std::min<long>((long)tiles_x * tiles_y * nchunks, std::min(3 * ctx->sms, RED_BLOCKS));
         if (ctx->packed) {
-            AC_CUDA(cudaFuncSetAttribute(ac::reduce_tma_kernel<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         ac::RQ_SMEM_BYTES));
             ac::reduce_tma_kernel<T, 2><<<blocks, ac::RQ_THREADS, ac::RQ_SMEM_BYTES, ctx->stream>>>(
                 a, ctx->map_a[ctx->cur], ctx->map_p[ctx->cur], tiles_x, tiles_y, nchunks);
         } else {
-            AC_CUDA(cudaFuncSetAttribute(ac::reduce_tma_kernel<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         ac::RQ_SMEM_BYTES));
             ac::reduce_tma_kernel<T, 1><<<blocks, ac::RQ_THREADS, ac::RQ_SMEM_BYTES, ctx->stream>>>(
                 a, ctx->map_a[ctx->cur], ctx->map_p[ctx->cur], tiles_x, tiles_y, nchunks);
         }
@@ -430,7 +439,6 @@ int reduce_t(ac_ctx* ctx, ac_diag* out) {
         const int nchunks = (L.nz + ac::RED_CZ - 1) / ac::RED_CZ;
         blocks = (int)std::min<long>((long)tiles_x * tiles_y * nchunks, RED_BLOCKS);
         const int sm = ac::red_smem_bytes<T, 1>();
-        AC_CUDA(cudaFuncSetAttribute(ac::reduce_stage1_kernel<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
         ac::reduce_stage1_kernel<T, 1><<<blocks, ac::RED_THREADS, sm, ctx->stream>>>(a, tiles_x, tiles_y, nchunks);
     }
     ac::reduce_stage2_kernel<<<1, 256, 0, ctx->stream>>>(a.partial, blocks, result);
@@ -455,11 +463,50 @@ int reduce_t(ac_ctx* ctx, ac_diag* out) {
     return AC_OK;
 }
 
+// extended diagnostics (diag_ext.cuh); the per-block partials live in the idle state buffer
+template <typename T>
+int reduce_ext_t(ac_ctx* ctx, double raw[3]) {
+    const ac::Layout& L = ctx->L;
+    ac::DiagExtArgs<T> a;
+    a.L = L;
+    fill_coeffs<T>(ctx, a.c);
+    for (int i = 0; i < 3; i++) a.bext[i] = (T)ctx->bext[i];
+    a.mixed_tensor = ctx->mixed;
+    for (int q = 0; q < AC_NFIELDS; q++) a.in[q] = ctx->field_ptr(ctx->cur, q);
+    a.partial = (ac::ExtVals*)ctx->field_ptr(1 - ctx->cur, 0);
+    ac::ExtVals* result = (ac::ExtVals*)(ctx->ws + ctx->cv.result_off + 128);
+    dim3 blk(32, 4, 2);
+    dim3 grd((L.nx + blk.x - 1) / blk.x, (L.ny + blk.y - 1) / blk.y, (L.nz + blk.z - 1) / blk.z);
+    const long nblocks = (long)grd.x * grd.y * grd.z;
+    if ((size_t)nblocks * sizeof(ac::ExtVals) > ctx->cv.field_bytes) return AC_ENOMEM;
+    if (ctx->packed)
+        ac::diag_ext_kernel<T, 2><<<grd, blk, 0, ctx->stream>>>(a);
+    else
+        ac::diag_ext_kernel<T, 1><<<grd, blk, 0, ctx->stream>>>(a);
+    ac::diag_ext_stage2_kernel<<<1, 256, 0, ctx->stream>>>(a.partial, nblocks, result);
+    ctx->launches += 2;
+    AC_CUDA(cudaGetLastError());
+    ac::ExtVals* host = (ac::ExtVals*)((char*)ctx->host_result + 64);
+    AC_CUDA(cudaMemcpyAsync(host, result, sizeof(ac::ExtVals), cudaMemcpyDeviceToHost, ctx->stream));
+    AC_CUDA(cudaStreamSynchronize(ctx->stream));
+    raw[0] = host->hk;
+    raw[1] = host->hc;
+    raw[2] = host->va2;
+    return AC_OK;
+}
+
 // ----- Eq. 4-6 on the host -----------------------------------------------------------------------
 void cross(const double a[3], const double b[3], double o[3]) {
     o[0] = a[1] * b[2] - a[2] * b[1];
     o[1] = a[2] * b[0] - a[0] * b[2];
     o[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+bool forcing_ok(const ac_forcing* f) {
+    if (!f) return true;
+    for (int i = 0; i < 3; i++)
+        if (!std::isfinite(f->k[i]) || !std::isfinite(f->re[i]) || !std::isfinite(f->im[i])) return false;
+    return std::isfinite(f->phase);
 }
 
 uint64_t splitmix64(uint64_t x) {
@@ -513,6 +560,23 @@ int configure(ac_ctx* ctx) {
     ctx->loaded = false;
     ctx->loaded_mask = 0;
     ctx->cur = 0;
+    ctx->next_substep = 0;
+    {
+        // opt-in shared-memory sizes of the reduction kernels, once per configuration
+        cudaError_t e = cudaSuccess;
+        if (ctx->dtype == AC_F64) {
+            e = cudaFuncSetAttribute(ac::reduce_tma_kernel<double, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, ac::RQ_SMEM_BYTES);
+            if (e == cudaSuccess)
+                e = cudaFuncSetAttribute(ac::reduce_stage1_kernel<double, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         ac::red_smem_bytes<double, 1>());
+        } else {
+            e = cudaFuncSetAttribute(ac::reduce_tma_kernel<float, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, ac::RQ_SMEM_BYTES);
+            if (e == cudaSuccess)
+                e = cudaFuncSetAttribute(ac::reduce_stage1_kernel<float, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         ac::red_smem_bytes<float, 1>());
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(reduction smem)");
+    }
     if (!ctx->march) return AC_OK;
     for (int b = 0; b < 2; b++) {
         int rc = make_state_map(&ctx->map_in[b], ctx->field_ptr(b, 0), ctx->L, ac::M_WX, ac::M_WY);
@@ -542,8 +606,7 @@ int configure(ac_ctx* ctx) {
     const int nzp = ctx->L.nz;
     const int tile_x = ctx->variant == 0 ? ac::Q_TX : ac::M_TX, tile_y = ctx->variant == 0 ? ac::Q_TY : ac::M_TY;
     const long tiles = (long)((ctx->L.nx + tile_x - 1) / tile_x) * ((ctx->L.ny + tile_y - 1) / tile_y);
-    int sms = 148;
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
+    const int sms = ctx->sms;
     long best_cost = -1;
     int best_n = 1;
     for (int n = 1; n <= 64; n++) {
@@ -560,10 +623,6 @@ int configure(ac_ctx* ctx) {
         }
     }
     ctx->nchunks = best_n;
-    if (const char* e = getenv("AC_MARCH_CZ")) {
-        ctx->cz = std::min(ac::M_CZMAX, std::max(1, atoi(e)));
-        ctx->nchunks = (nzp + ctx->cz - 1) / ctx->cz;
-    }
     return AC_OK;
 }
 
@@ -611,6 +670,9 @@ int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double
     ctx->host_result = nullptr;
     ctx->cz = 0;
     ctx->nchunks = 1;
+    ctx->device = dev;
+    ctx->sms = prop.multiProcessorCount;
+    ctx->next_substep = 0;
     if (workspace_dev) {
         ctx->ws = (char*)workspace_dev;
         ctx->owns_ws = false;
@@ -627,7 +689,7 @@ int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double
     }
     int rc = configure(ctx);
     if (rc == AC_OK) {
-        cudaError_t e = cudaMallocHost((void**)&ctx->host_result, sizeof(ac::RedVals));
+        cudaError_t e = cudaMallocHost((void**)&ctx->host_result, 128);   // RedVals at 0, ExtVals at 64
         if (e != cudaSuccess) rc = cuda_fail(e, "cudaMallocHost");
     }
     if (rc != AC_OK) {
@@ -640,12 +702,14 @@ int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double
 }
 
 int ac_load_state(ac_ctx* ctx, const void* const fields[AC_NFIELDS], int src_on_device) {
+    DeviceGuard guard(ctx);
     if (!ctx || !fields) return AC_EINVAL;
     for (int q = 0; q < AC_NFIELDS; q++)
         if (!fields[q]) return AC_EINVAL;
     ctx->cur = 0;
     ctx->loaded = false;
     ctx->loaded_mask = 0;
+    ctx->next_substep = 0;          // a whole new state starts a new step
     for (int q = 0; q < AC_NFIELDS; q++) {
         const int rc = ac_load_field(ctx, q, fields[q], src_on_device);
         if (rc != AC_OK) return rc;
@@ -654,7 +718,11 @@ int ac_load_state(ac_ctx* ctx, const void* const fields[AC_NFIELDS], int src_on_
 }
 
 int ac_load_field(ac_ctx* ctx, int q, const void* field, int src_on_device) {
+    DeviceGuard guard(ctx);
     if (!ctx || !field || q < 0 || q >= AC_NFIELDS) return AC_EINVAL;
+    // inside a step the idle buffer holds the previous state (2N register): nothing may be staged there, and
+    // replacing a field of the current state would corrupt the register as well
+    if (ctx->next_substep != 0) return AC_ESTATE;
     const int rc = ctx->dtype == AC_F64 ? load_field_t<double>(ctx, ctx->cur, q, field, src_on_device)
                                         : load_field_t<float>(ctx, ctx->cur, q, field, src_on_device);
     if (rc != AC_OK) return rc;
@@ -664,10 +732,12 @@ int ac_load_field(ac_ctx* ctx, int q, const void* field, int src_on_device) {
 }
 
 int ac_store_state(ac_ctx* ctx, void* const fields[AC_NFIELDS], int dst_on_device) {
+    DeviceGuard guard(ctx);
     if (!ctx || !fields) return AC_EINVAL;
     for (int q = 0; q < AC_NFIELDS; q++)
         if (!fields[q]) return AC_EINVAL;
     if (!ctx->loaded) return AC_ESTATE;
+    if (!dst_on_device && ctx->next_substep != 0) return AC_ESTATE;   // the host path stages in the idle buffer
     for (int q = 0; q < AC_NFIELDS; q++) {
         const int rc = ctx->dtype == AC_F64 ? store_field_t<double>(ctx, q, fields[q], dst_on_device)
                                             : store_field_t<float>(ctx, q, fields[q], dst_on_device);
@@ -678,8 +748,10 @@ int ac_store_state(ac_ctx* ctx, void* const fields[AC_NFIELDS], int dst_on_devic
 }
 
 int ac_store_field(ac_ctx* ctx, int q, void* field, int dst_on_device) {
+    DeviceGuard guard(ctx);
     if (!ctx || !field || q < 0 || q >= AC_NFIELDS) return AC_EINVAL;
     if (!ctx->loaded) return AC_ESTATE;
+    if (!dst_on_device && ctx->next_substep != 0) return AC_ESTATE;
     const int rc = ctx->dtype == AC_F64 ? store_field_t<double>(ctx, q, field, dst_on_device)
                                         : store_field_t<float>(ctx, q, field, dst_on_device);
     if (rc != AC_OK) return rc;
@@ -688,23 +760,24 @@ int ac_store_field(ac_ctx* ctx, int q, void* field, int dst_on_device) {
 }
 
 int ac_step(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
+    DeviceGuard guard(ctx);
     if (!ctx) return AC_EINVAL;
     if (!(dt > 0.0) || !std::isfinite(dt)) return AC_EINVAL;
-    if (!ctx->loaded) return AC_ESTATE;
-    if (forcing) {
-        for (int i = 0; i < 3; i++)
-            if (!std::isfinite(forcing->k[i]) || !std::isfinite(forcing->re[i]) || !std::isfinite(forcing->im[i]))
-                return AC_EINVAL;
-        if (!std::isfinite(forcing->phase)) return AC_EINVAL;
-    }
+    if (!forcing_ok(forcing)) return AC_EINVAL;
+    if (!ctx->loaded || ctx->next_substep != 0) return AC_ESTATE;
     return ctx->dtype == AC_F64 ? step_t<double>(ctx, dt, forcing) : step_t<float>(ctx, dt, forcing);
 }
 
 int ac_substep(ac_ctx* ctx, int s, double dt, const ac_forcing* forcing) {
+    DeviceGuard guard(ctx);
     if (!ctx || s < 0 || s > 2) return AC_EINVAL;
     if (!(dt > 0.0) || !std::isfinite(dt)) return AC_EINVAL;
+    if (!forcing_ok(forcing)) return AC_EINVAL;
     if (!ctx->loaded) return AC_ESTATE;
-    return ctx->dtype == AC_F64 ? step_t<double>(ctx, dt, forcing, s, s + 1) : step_t<float>(ctx, dt, forcing, s, s + 1);
+    if (s != ctx->next_substep) return AC_ESTATE;      // substeps run in order 0, 1, 2: the 2N register is the buffers' difference
+    const int rc = ctx->dtype == AC_F64 ? step_t<double>(ctx, dt, forcing, s, s + 1) : step_t<float>(ctx, dt, forcing, s, s + 1);
+    if (rc == AC_OK) ctx->next_substep = (s + 1) % 3;
+    return rc;
 }
 
 int ac_state_layout(const ac_ctx* ctx, ac_layout_info* out) {
@@ -727,12 +800,14 @@ void* ac_field_device_ptr(ac_ctx* ctx, int q) {
 }
 
 int ac_reduce(ac_ctx* ctx, ac_diag* out) {
+    DeviceGuard guard(ctx);
     if (!ctx || !out) return AC_EINVAL;
     if (!ctx->loaded) return AC_ESTATE;
     return ctx->dtype == AC_F64 ? reduce_t<double>(ctx, out) : reduce_t<float>(ctx, out);
 }
 
 int ac_reduce_raw(ac_ctx* ctx, double out[6]) {
+    DeviceGuard guard(ctx);
     if (!ctx || !out) return AC_EINVAL;
     if (!ctx->loaded) return AC_ESTATE;
     ac_diag d;
@@ -745,6 +820,37 @@ int ac_reduce_raw(ac_ctx* ctx, double out[6]) {
     out[3] = r.mb;
     out[4] = r.lmin;
     out[5] = r.lmax;
+    return AC_OK;
+}
+
+int ac_reduce_ext_raw(ac_ctx* ctx, double out[3]) {
+    DeviceGuard guard(ctx);
+    if (!ctx || !out) return AC_EINVAL;
+    if (!ctx->loaded || ctx->next_substep != 0) return AC_ESTATE;    // the partials are staged in the idle buffer
+    return ctx->dtype == AC_F64 ? reduce_ext_t<double>(ctx, out) : reduce_ext_t<float>(ctx, out);
+}
+
+int ac_reduce_ext(ac_ctx* ctx, ac_diag_ext* out) {
+    if (!ctx || !out) return AC_EINVAL;
+    if (!ctx->loaded || ctx->next_substep != 0) return AC_ESTATE;
+    ac_diag d;
+    int rc = ac_reduce(ctx, &d);
+    if (rc != AC_OK) return rc;
+    double raw[3];
+    rc = ac_reduce_ext_raw(ctx, raw);
+    if (rc != AC_OK) return rc;
+    const ac_grid& g = ctx->grid;
+    const double ncell = (double)g.nx * g.ny * g.nz;
+    out->kin_hel = raw[0] / ncell;
+    out->cur_hel = raw[1] / ncell;
+    out->va_max = std::sqrt(raw[2]);
+    out->nonfinite = d.nonfinite || !(std::isfinite(raw[0]) && std::isfinite(raw[1]) && std::isfinite(raw[2]));
+    // G15 with the Alfven term: the signal speed c_s becomes sqrt(c_s^2 + max v_A^2)
+    const double hmin = std::min(g.lx / g.nx, std::min(g.ly / g.ny, g.lz / g.nz));
+    double dt = ctx->c_u * hmin / (d.umax + std::sqrt(ctx->cs * ctx->cs + raw[2]));
+    const double dd = std::max(ctx->nu, ctx->eta);
+    if (dd > 0.0) dt = std::min(dt, ctx->c_nu * hmin * hmin / dd);
+    out->dt_cfl_alfven = dt;
     return AC_OK;
 }
 
@@ -839,6 +945,7 @@ int ac_set_upwind(ac_ctx* ctx, int on) {
 }
 
 int ac_set_mixed(ac_ctx* ctx, int mode) {
+    DeviceGuard guard(ctx);
     if (!ctx || (mode != 0 && mode != 1)) return AC_EINVAL;
     if (mode == ctx->mixed) return AC_OK;
     // the tensor-product reading exists in the direct kernel only, whose fp32 device layout differs
@@ -848,6 +955,7 @@ int ac_set_mixed(ac_ctx* ctx, int mode) {
 }
 
 int ac_set_variant(ac_ctx* ctx, int variant) {
+    DeviceGuard guard(ctx);
     if (!ctx) return AC_EINVAL;
     if (variant < 0 || variant > 2) return AC_EINVAL;
     if (variant == ctx->variant) return AC_OK;
@@ -861,6 +969,7 @@ long long ac_launch_count(const ac_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 void ac_free(ac_ctx* ctx) {
     if (!ctx) return;
+    DeviceGuard guard(ctx);
     cudaStreamSynchronize(ctx->stream);
     if (ctx->owns_ws) cudaFree(ctx->ws);
     if (ctx->host_result) cudaFreeHost(ctx->host_result);
