@@ -128,9 +128,8 @@ int ac_step(ac_ctx* ctx, double dt, const ac_forcing* forcing);
  * (ac_state_layout; element (x, y, z) of field q at ac_field_device_ptr(ctx, q) + (x + gx) + pitch * (y + 3) +
  * plane_elems * (z + 3) elements) the planes to send, [nz_local, nz_local + 3) upwards and [3, 6) downwards, and the
  * planes to receive, [0, 3) and [nz_local + 3, nz_local + 6), are contiguous blocks of 3 * plane_elems elements per
- * field, so the exchange is 2 x 7 plain copies (peer copies, ncclSend/ncclRecv, torch.distributed) and needs no
- * pack kernel.  The forcing phase of a rank is the global phase + k_z * z0 with z0 the position of its first plane.
- * Only layouts with packed_pairs == 0 can be exchanged this way (fp64, or fp32 with ac_set_variant(ctx, 1)).
+ * field, so the exchange can be 2 x 7 plain copies (layouts with packed_pairs == 0 only); ac_halo_pack /
+ * ac_halo_unpack below do the same through two dense buffers for every layout, packed fp32 pairs included.
  * ac_substep: substep s = 0, 1, 2 of the 2N-RK3 step; three calls with the same dt and forcing equal ac_step.
  *   The substeps must come in order (AC_ESTATE otherwise; ac_load_state restarts at 0): between substeps the idle
  *   state buffer holds the previous state, from which the 2N register is rebuilt.  Therefore, after substep 0 or 1,
@@ -145,6 +144,34 @@ typedef struct {
     size_t plane_elems, field_elems;
 } ac_layout_info;
 int ac_substep(ac_ctx* ctx, int s, double dt, const ac_forcing* forcing);
+
+/* ---- the slab as the paper runs it ("it is critical to carry out computations in parallel with
+ * communication", the six functions of a substep PAPER.md:153-158, Fig. 3) -------------------------------------
+ * ac_set_slab: declares the context a slab of a global grid of nz_global planes whose first plane is z0_plane
+ *   (nz_global == nz: an ordinary periodic box again).  From then on: the forcing of ac_step / ac_substep* is the
+ *   GLOBAL wave (the slab adds k_z z0 to the phase itself) and ac_make_forcing / ac_forcing_from_draws take the
+ *   global box length for k; the substep kernels leave the z ghost planes to ac_halo_unpack.
+ * ac_substep_part: substep s in two launches.  AC_PART_INNER updates the planes [3, nz - 3), which read no z ghost
+ *   plane and can therefore run while the halo of the current state is still in flight; AC_PART_OUTER updates the
+ *   3 + 3 boundary planes (after ac_halo_unpack), refreshes the x / y ghost zones and swaps the buffers.  INNER
+ *   then OUTER equal ac_substep bit for bit.  Errors as ac_substep; AC_ESTATE for OUTER without INNER or twice.
+ * ac_halo_bytes: size of ONE halo buffer, 7 fields x 3 planes x (my * pitch) cells of the context's dtype.
+ * ac_halo_pack: the 3 bottom planes of cells of the CURRENT state (all fields, x / y ghost zones included) into
+ *   send_lo (for the rank below: its upper ghost planes) and the 3 top planes into send_hi (for the rank above),
+ *   dense [7][3][my * pitch]; works for packed fp32 pairs too (it picks the lanes).  ac_halo_unpack: recv_lo (the
+ *   top planes of the rank below) into the ghost planes below, recv_hi into those above.  Both run on cuda_stream
+ *   (NULL: the context's stream) so that a caller can keep the exchange on a second stream; the caller orders them
+ *   against the substeps with events: pack after the previous OUTER / ac_substep, unpack before the next OUTER.
+ * ac_diag_combine: the diagnostics of the whole box from nranks ac_reduce_raw results (raws[6 * nranks], folded in
+ *   rank order: sum, max, sum, max, min, max) with the context's CFL constants; pure host arithmetic. */
+#define AC_PART_INNER 1
+#define AC_PART_OUTER 2
+int ac_set_slab(ac_ctx* ctx, int z0_plane, int nz_global);
+int ac_substep_part(ac_ctx* ctx, int s, double dt, const ac_forcing* forcing, int part);
+size_t ac_halo_bytes(const ac_ctx* ctx);
+int ac_halo_pack(ac_ctx* ctx, void* send_lo_dev, void* send_hi_dev, void* cuda_stream);
+int ac_halo_unpack(ac_ctx* ctx, const void* recv_lo_dev, const void* recv_hi_dev, void* cuda_stream);
+int ac_diag_combine(const ac_ctx* ctx, const double* raws, int nranks, ac_diag* out);
 int ac_state_layout(const ac_ctx* ctx, ac_layout_info* out);
 void* ac_field_device_ptr(ac_ctx* ctx, int q);
 int ac_reduce_raw(ac_ctx* ctx, double out[6]);

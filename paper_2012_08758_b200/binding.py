@@ -13,13 +13,15 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libac_mhd.so")
 
 AC_F32, AC_F64 = 0, 1
+AC_PART_INNER, AC_PART_OUTER = 1, 2
 NFIELDS = 7
 EXPORTS = (
     "ac_workspace_bytes", "ac_init", "ac_load_state", "ac_store_state", "ac_load_field", "ac_store_field", "ac_step",
     "ac_reduce",
     "ac_forcing_from_draws", "ac_forcing_params", "ac_make_forcing", "ac_set_bext", "ac_set_cfl", "ac_set_variant",
     "ac_set_upwind", "ac_set_mixed", "ac_substep", "ac_state_layout", "ac_field_device_ptr", "ac_reduce_raw",
-    "ac_reduce_ext", "ac_reduce_ext_raw",
+    "ac_reduce_ext", "ac_reduce_ext_raw", "ac_set_slab", "ac_substep_part", "ac_halo_bytes", "ac_halo_pack",
+    "ac_halo_unpack", "ac_diag_combine",
     "ac_launch_count", "ac_free", "ac_strerror", "ac_version",
 )
 
@@ -119,6 +121,18 @@ def load_library():
     L.ac_reduce_ext.restype = i32
     L.ac_reduce_ext_raw.argtypes = [vp, ctypes.POINTER(dbl)]
     L.ac_reduce_ext_raw.restype = i32
+    L.ac_set_slab.argtypes = [vp, i32, i32]
+    L.ac_set_slab.restype = i32
+    L.ac_substep_part.argtypes = [vp, i32, dbl, ctypes.POINTER(AcForcing), i32]
+    L.ac_substep_part.restype = i32
+    L.ac_halo_bytes.argtypes = [vp]
+    L.ac_halo_bytes.restype = ctypes.c_size_t
+    L.ac_halo_pack.argtypes = [vp, vp, vp, vp]
+    L.ac_halo_pack.restype = i32
+    L.ac_halo_unpack.argtypes = [vp, vp, vp, vp]
+    L.ac_halo_unpack.restype = i32
+    L.ac_diag_combine.argtypes = [vp, ctypes.POINTER(dbl), i32, ctypes.POINTER(AcDiag)]
+    L.ac_diag_combine.restype = i32
     L.ac_launch_count.argtypes = [vp]
     L.ac_launch_count.restype = ctypes.c_longlong
     L.ac_free.argtypes = [vp]
@@ -267,6 +281,35 @@ class Context:
             f = forcing if isinstance(forcing, AcForcing) else AcForcing.from_tuple(forcing)
         _check(self._lib.ac_substep(self._ctx, int(s), float(dt), ctypes.byref(f) if f is not None else None),
                "ac_substep")
+
+    def ac_substep_part(self, s, dt, forcing, part):
+        f = None
+        if forcing is not None:
+            f = forcing if isinstance(forcing, AcForcing) else AcForcing.from_tuple(forcing)
+        _check(self._lib.ac_substep_part(self._ctx, int(s), float(dt), ctypes.byref(f) if f is not None else None,
+                                         int(part)), "ac_substep_part")
+
+    def ac_set_slab(self, z0_plane, nz_global):
+        _check(self._lib.ac_set_slab(self._ctx, int(z0_plane), int(nz_global)), "ac_set_slab")
+
+    def ac_halo_bytes(self):
+        return int(self._lib.ac_halo_bytes(self._ctx))
+
+    def ac_halo_pack(self, send_lo, send_hi, stream=None):
+        """send_lo / send_hi: device tensors of ac_halo_bytes() bytes each; stream: a torch stream or None."""
+        _check(self._lib.ac_halo_pack(self._ctx, ctypes.c_void_p(send_lo.data_ptr()), ctypes.c_void_p(send_hi.data_ptr()),
+                                      ctypes.c_void_p(stream.cuda_stream if stream is not None else 0)), "ac_halo_pack")
+
+    def ac_halo_unpack(self, recv_lo, recv_hi, stream=None):
+        _check(self._lib.ac_halo_unpack(self._ctx, ctypes.c_void_p(recv_lo.data_ptr()), ctypes.c_void_p(recv_hi.data_ptr()),
+                                        ctypes.c_void_p(stream.cuda_stream if stream is not None else 0)), "ac_halo_unpack")
+
+    def ac_diag_combine(self, raws):
+        """raws: sequence of ac_reduce_raw tuples, one per rank, in rank order."""
+        flat = (ctypes.c_double * (6 * len(raws)))(*[float(v) for r in raws for v in r])
+        d = AcDiag()
+        _check(self._lib.ac_diag_combine(self._ctx, flat, len(raws), ctypes.byref(d)), "ac_diag_combine")
+        return d.as_dict()
 
     def ac_state_layout(self):
         info = AcLayoutInfo()

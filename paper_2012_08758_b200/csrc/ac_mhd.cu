@@ -166,6 +166,9 @@ struct ac_ctx {
     CUtensorMap map_qprev[2];  // and interior-tile boxes
     int cz, nchunks;           // z chunking of the march kernel
     int device, sms;           // CUDA device ordinal of the context and its SM count
+    bool slab;                 // a z slab of a larger box (ac_set_slab): neighbours own the z ghost planes
+    int z0_plane, nz_global;   // index of the slab's first plane in the global grid, planes of the global grid
+    int inner_done;            // substep whose inner part has been launched (-1: none)
     int next_substep;          // 0 between full steps; 1, 2 inside a step driven by ac_substep (the idle buffer is live then)
 
     void* field_ptr(int buf, int q) const { return ws + ((size_t)buf * AC_NFIELDS + q) * cv.field_bytes; }
@@ -320,18 +323,37 @@ void fill_march_coef(const ac_ctx* ctx, ac::MarchCoef<E>& c, double dt, int s, c
     c.rk_b = S::of(RK_BETA[s] * dt);
 }
 
-// substeps [s_begin, s_end) of one RK3 step (ac_step: 0..3; ac_substep: one)
+// which planes of the slab a launch updates (AC_PART_* of the header)
+enum { PART_ALL = 0, PART_INNER = 1, PART_OUTER = 2 };
+
+// One substep s, or its inner / outer part.  INNER = planes [3, nz - 3): they read no z ghost plane, so they can run
+// while the halo exchange is in flight (Fig. 3).  OUTER = the 3 + 3 boundary planes, then the
+// ghost zones of the new state and the buffer swap.  ALL = both in one launch.
 template <typename T>
-int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s_begin = 0, int s_end = 3) {
+int substep_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s, int part) {
     const ac::Layout& L = ctx->L;
     const ac_grid& g = ctx->grid;
     T* ftab = (T*)(ctx->ws + ctx->cv.ftab_off);
-    if (forcing) {
+    if (forcing && part != PART_OUTER) {
+        // a slab sees the global wave with its own origin: phase + k_z z0 (Eq. 4)
+        const double hz = g.lz / g.nz;
+        const double phase = forcing->phase + forcing->k[2] * (ctx->z0_plane * hz);
         const int n = g.nx + g.ny + g.nz;
         ac::forcing_tables_kernel<T><<<(n + 255) / 256, 256, 0, ctx->stream>>>(
-            ftab, g.nx, g.ny, g.nz, forcing->k[0], forcing->k[1], forcing->k[2], g.lx / g.nx, g.ly / g.ny, g.lz / g.nz,
-            forcing->phase);
+            ftab, g.nx, g.ny, g.nz, forcing->k[0], forcing->k[1], forcing->k[2], g.lx / g.nx, g.ly / g.ny, hz, phase);
         ctx->launches++;
+    }
+    // plane ranges of this part, in storage planes (packed fp32: the boundary cells sit in the first and last 3 pairs)
+    const int nzs = L.nz;
+    const bool split = nzs > 2 * ac::R;
+    int nr = 0, r0[2], r1[2];
+    if (part == PART_ALL || (part == PART_OUTER && !split)) {
+        r0[nr] = 0, r1[nr] = nzs, nr++;
+    } else if (part == PART_INNER) {
+        if (split) r0[nr] = ac::R, r1[nr] = nzs - ac::R, nr++;
+    } else {
+        r0[nr] = 0, r1[nr] = ac::R, nr++;
+        r0[nr] = nzs - ac::R, r1[nr] = nzs, nr++;
     }
     if (ctx->march) {
         using E = typename ac::ElemOf<T>::E;
@@ -341,37 +363,44 @@ int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s_begin = 0, i
         a.nz_full = g.nz;
         a.cz = ctx->cz;
         a.has_forcing = forcing ? 1 : 0;
-        a.wrap_z = 1;
-        for (int s = s_begin; s < s_end; s++) {
-            a.substep = s;
-            fill_march_coef<E>(ctx, a.c, dt, s, forcing);
-            for (int q = 0; q < AC_NFIELDS; q++) a.out[q] = (E*)ctx->field_ptr(1 - ctx->cur, q);
-            dim3 grd((L.nx + ac::M_TX - 1) / ac::M_TX, (L.ny + ac::M_TY - 1) / ac::M_TY, ctx->nchunks);
+        a.wrap_z = ctx->slab ? 0 : 1;
+        a.substep = s;
+        fill_march_coef<E>(ctx, a.c, dt, s, forcing);
+        for (int q = 0; q < AC_NFIELDS; q++) a.out[q] = (E*)ctx->field_ptr(1 - ctx->cur, q);
+        for (int r = 0; r < nr; r++) {
+            a.z_begin = r0[r];
+            a.z_end = r1[r];
+            const int nch = (r1[r] - r0[r] + ctx->cz - 1) / ctx->cz;
             if (ctx->variant == 0) {
                 // pair-march: 16 x 16 tiles, a thread owns two cells
-                dim3 gq((L.nx + ac::Q_TX - 1) / ac::Q_TX, (L.ny + ac::Q_TY - 1) / ac::Q_TY, ctx->nchunks);
+                dim3 gq((L.nx + ac::Q_TX - 1) / ac::Q_TX, (L.ny + ac::Q_TY - 1) / ac::Q_TY, nch);
                 if (ctx->upwind)
                     ac::substep_pair_kernel<T, true><<<gq, ac::Q_THREADS, ac::Q_SMEM_BYTES, ctx->stream>>>(
                         a, ctx->map_qin[ctx->cur], ctx->map_qprev[1 - ctx->cur]);
                 else
                     ac::substep_pair_kernel<T, false><<<gq, ac::Q_THREADS, ac::Q_SMEM_BYTES, ctx->stream>>>(
                         a, ctx->map_qin[ctx->cur], ctx->map_qprev[1 - ctx->cur]);
-            } else if (ctx->upwind) {
-                ac::substep_march_kernel<T, true><<<grd, ac::M_THREADS, ac::M_SMEM_BYTES, ctx->stream>>>(
-                    a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
             } else {
-                ac::substep_march_kernel<T, false><<<grd, ac::M_THREADS, ac::M_SMEM_BYTES, ctx->stream>>>(
-                    a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
+                dim3 grd((L.nx + ac::M_TX - 1) / ac::M_TX, (L.ny + ac::M_TY - 1) / ac::M_TY, nch);
+                if (ctx->upwind)
+                    ac::substep_march_kernel<T, true><<<grd, ac::M_THREADS, ac::M_SMEM_BYTES, ctx->stream>>>(
+                        a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
+                else
+                    ac::substep_march_kernel<T, false><<<grd, ac::M_THREADS, ac::M_SMEM_BYTES, ctx->stream>>>(
+                        a, ctx->map_in[ctx->cur], ctx->map_prev[1 - ctx->cur]);
             }
             ctx->launches++;
-            // S1: refresh the ghost zones of the buffer just written
+        }
+        if (part != PART_INNER) {
+            // S1: refresh the ghost zones of the buffer just written.  The z ghost planes of a slab belong to its
+            // neighbours (ac_halo_unpack); of packed fp32 pairs one lane is the slab's own cell, so they are kept.
             const int nb_rows = 2 * ac::R * L.my + 2 * ac::R * L.nz;
             const int na_tasks = (int)(((long)L.ny * L.nz + ac::M_GHOST_ROWS_PER_TASK - 1) / ac::M_GHOST_ROWS_PER_TASK);
-            dim3 gg((unsigned)std::min(nb_rows + na_tasks, RED_BLOCKS), AC_NFIELDS, 1);
+            const int first_row = (ctx->slab && !ctx->packed) ? 2 * ac::R * L.my : 0;
+            dim3 gg((unsigned)std::min(nb_rows + na_tasks - first_row, RED_BLOCKS), AC_NFIELDS, 1);
             ac::ghost_fill_kernel<E><<<gg, ac::M_GHOST_THREADS, 0, ctx->stream>>>((E*)ctx->field_ptr(1 - ctx->cur, 0), L,
-                                                                              nb_rows, na_tasks);
+                                                                              nb_rows, na_tasks, first_row);
             ctx->launches++;
-            ctx->cur = 1 - ctx->cur;
         }
     } else {
         ac::SubstepArgs<T> a;
@@ -389,22 +418,34 @@ int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s_begin = 0, i
             a.p.fim[i] = forcing ? (T)forcing->im[i] : T(0);
         }
         a.ftab = ftab;
-        for (int s = s_begin; s < s_end; s++) {
-            a.p.substep = s;
-            a.p.rk_a = (s == 0) ? T(0) : (T)(RK_BETA[s] * RK_ALPHA[s] / RK_BETA[s - 1]);
-            a.p.rk_b = (T)(RK_BETA[s] * dt);
-            for (int q = 0; q < AC_NFIELDS; q++) {
-                a.in[q] = (const T*)ctx->field_ptr(ctx->cur, q);
-                a.out[q] = (T*)ctx->field_ptr(1 - ctx->cur, q);
-            }
+        a.p.substep = s;
+        a.p.rk_a = (s == 0) ? T(0) : (T)(RK_BETA[s] * RK_ALPHA[s] / RK_BETA[s - 1]);
+        a.p.rk_b = (T)(RK_BETA[s] * dt);
+        for (int q = 0; q < AC_NFIELDS; q++) {
+            a.in[q] = (const T*)ctx->field_ptr(ctx->cur, q);
+            a.out[q] = (T*)ctx->field_ptr(1 - ctx->cur, q);
+        }
+        for (int r = 0; r < nr; r++) {
+            a.z_begin = r0[r];
+            a.z_end = r1[r];
             dim3 blk(32, 4, 2);
-            dim3 grd((L.nx + blk.x - 1) / blk.x, (L.ny + blk.y - 1) / blk.y, (L.nz + blk.z - 1) / blk.z);
+            dim3 grd((L.nx + blk.x - 1) / blk.x, (L.ny + blk.y - 1) / blk.y, (r1[r] - r0[r] + blk.z - 1) / blk.z);
             ac::substep_direct_kernel<T><<<grd, blk, 0, ctx->stream>>>(a);
             ctx->launches++;
-            ctx->cur = 1 - ctx->cur;
         }
     }
+    if (part != PART_INNER) ctx->cur = 1 - ctx->cur;
     AC_CUDA(cudaGetLastError());
+    return AC_OK;
+}
+
+// substeps [s_begin, s_end) of one RK3 step (ac_step: 0..3; ac_substep: one)
+template <typename T>
+int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s_begin = 0, int s_end = 3) {
+    for (int s = s_begin; s < s_end; s++) {
+        const int rc = substep_t<T>(ctx, dt, forcing, s, PART_ALL);
+        if (rc != AC_OK) return rc;
+    }
     return AC_OK;
 }
 
@@ -673,6 +714,10 @@ int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double
     ctx->device = dev;
     ctx->sms = prop.multiProcessorCount;
     ctx->next_substep = 0;
+    ctx->slab = false;
+    ctx->z0_plane = 0;
+    ctx->nz_global = grid->nz;
+    ctx->inner_done = -1;
     if (workspace_dev) {
         ctx->ws = (char*)workspace_dev;
         ctx->owns_ws = false;
@@ -710,6 +755,7 @@ int ac_load_state(ac_ctx* ctx, const void* const fields[AC_NFIELDS], int src_on_
     ctx->loaded = false;
     ctx->loaded_mask = 0;
     ctx->next_substep = 0;          // a whole new state starts a new step
+    ctx->inner_done = -1;
     for (int q = 0; q < AC_NFIELDS; q++) {
         const int rc = ac_load_field(ctx, q, fields[q], src_on_device);
         if (rc != AC_OK) return rc;
@@ -764,7 +810,7 @@ int ac_step(ac_ctx* ctx, double dt, const ac_forcing* forcing) {
     if (!ctx) return AC_EINVAL;
     if (!(dt > 0.0) || !std::isfinite(dt)) return AC_EINVAL;
     if (!forcing_ok(forcing)) return AC_EINVAL;
-    if (!ctx->loaded || ctx->next_substep != 0) return AC_ESTATE;
+    if (!ctx->loaded || ctx->next_substep != 0 || ctx->inner_done != -1) return AC_ESTATE;
     return ctx->dtype == AC_F64 ? step_t<double>(ctx, dt, forcing) : step_t<float>(ctx, dt, forcing);
 }
 
@@ -774,10 +820,113 @@ int ac_substep(ac_ctx* ctx, int s, double dt, const ac_forcing* forcing) {
     if (!(dt > 0.0) || !std::isfinite(dt)) return AC_EINVAL;
     if (!forcing_ok(forcing)) return AC_EINVAL;
     if (!ctx->loaded) return AC_ESTATE;
-    if (s != ctx->next_substep) return AC_ESTATE;      // substeps run in order 0, 1, 2: the 2N register is the buffers' difference
+    if (s != ctx->next_substep || ctx->inner_done != -1) return AC_ESTATE;   // substeps run in order 0, 1, 2: the 2N register is the buffers' difference
     const int rc = ctx->dtype == AC_F64 ? step_t<double>(ctx, dt, forcing, s, s + 1) : step_t<float>(ctx, dt, forcing, s, s + 1);
     if (rc == AC_OK) ctx->next_substep = (s + 1) % 3;
     return rc;
+}
+
+int ac_substep_part(ac_ctx* ctx, int s, double dt, const ac_forcing* forcing, int part) {
+    DeviceGuard guard(ctx);
+    if (!ctx || s < 0 || s > 2 || (part != AC_PART_INNER && part != AC_PART_OUTER)) return AC_EINVAL;
+    if (!(dt > 0.0) || !std::isfinite(dt)) return AC_EINVAL;
+    if (!forcing_ok(forcing)) return AC_EINVAL;
+    if (!ctx->loaded || s != ctx->next_substep) return AC_ESTATE;
+    if (part == AC_PART_INNER ? ctx->inner_done != -1 : ctx->inner_done != s) return AC_ESTATE;   // inner first, once
+    const int rc = ctx->dtype == AC_F64 ? substep_t<double>(ctx, dt, forcing, s, part == AC_PART_INNER ? PART_INNER : PART_OUTER)
+                                        : substep_t<float>(ctx, dt, forcing, s, part == AC_PART_INNER ? PART_INNER : PART_OUTER);
+    if (rc != AC_OK) return rc;
+    if (part == AC_PART_INNER) {
+        ctx->inner_done = s;
+    } else {
+        ctx->inner_done = -1;
+        ctx->next_substep = (s + 1) % 3;
+    }
+    return AC_OK;
+}
+
+int ac_set_slab(ac_ctx* ctx, int z0_plane, int nz_global) {
+    if (!ctx) return AC_EINVAL;
+    if (nz_global < ctx->grid.nz || z0_plane < 0 || z0_plane + ctx->grid.nz > nz_global) return AC_EINVAL;
+    if (ctx->next_substep != 0 || ctx->inner_done != -1) return AC_ESTATE;
+    ctx->slab = nz_global != ctx->grid.nz;
+    ctx->z0_plane = z0_plane;
+    ctx->nz_global = nz_global;
+    return AC_OK;
+}
+
+size_t ac_halo_bytes(const ac_ctx* ctx) {
+    if (!ctx) return 0;
+    return (size_t)AC_NFIELDS * ac::R * ctx->L.plane * elem_size(ctx->dtype);
+}
+
+int ac_halo_pack(ac_ctx* ctx, void* send_lo_dev, void* send_hi_dev, void* cuda_stream) {
+    DeviceGuard guard(ctx);
+    if (!ctx || !send_lo_dev || !send_hi_dev) return AC_EINVAL;
+    if (!ctx->loaded || ctx->inner_done != -1) return AC_ESTATE;
+    cudaStream_t st = cuda_stream ? (cudaStream_t)cuda_stream : ctx->stream;
+    const ac::Layout& L = ctx->L;
+    const size_t per_field = (size_t)ac::R * L.plane;
+    dim3 grd((unsigned)((per_field + 255) / 256), AC_NFIELDS, 1);
+    void* state = ctx->field_ptr(ctx->cur, 0);
+    if (ctx->dtype == AC_F64)
+        ac::halo_pack_kernel<double, 1><<<grd, 256, 0, st>>>(state, L.field, L, (double*)send_lo_dev, (double*)send_hi_dev);
+    else if (ctx->packed)
+        ac::halo_pack_kernel<float, 2><<<grd, 256, 0, st>>>(state, L.field, L, (float*)send_lo_dev, (float*)send_hi_dev);
+    else
+        ac::halo_pack_kernel<float, 1><<<grd, 256, 0, st>>>(state, L.field, L, (float*)send_lo_dev, (float*)send_hi_dev);
+    ctx->launches++;
+    AC_CUDA(cudaGetLastError());
+    return AC_OK;
+}
+
+int ac_halo_unpack(ac_ctx* ctx, const void* recv_lo_dev, const void* recv_hi_dev, void* cuda_stream) {
+    DeviceGuard guard(ctx);
+    if (!ctx || !recv_lo_dev || !recv_hi_dev) return AC_EINVAL;
+    if (!ctx->loaded) return AC_ESTATE;
+    cudaStream_t st = cuda_stream ? (cudaStream_t)cuda_stream : ctx->stream;
+    const ac::Layout& L = ctx->L;
+    const size_t per_field = (size_t)ac::R * L.plane;
+    dim3 grd((unsigned)((per_field + 255) / 256), AC_NFIELDS, 1);
+    void* state = ctx->field_ptr(ctx->cur, 0);
+    if (ctx->dtype == AC_F64)
+        ac::halo_unpack_kernel<double, 1><<<grd, 256, 0, st>>>(state, L.field, L, (const double*)recv_lo_dev, (const double*)recv_hi_dev);
+    else if (ctx->packed)
+        ac::halo_unpack_kernel<float, 2><<<grd, 256, 0, st>>>(state, L.field, L, (const float*)recv_lo_dev, (const float*)recv_hi_dev);
+    else
+        ac::halo_unpack_kernel<float, 1><<<grd, 256, 0, st>>>(state, L.field, L, (const float*)recv_lo_dev, (const float*)recv_hi_dev);
+    ctx->launches++;
+    AC_CUDA(cudaGetLastError());
+    return AC_OK;
+}
+
+int ac_diag_combine(const ac_ctx* ctx, const double* raws, int nranks, ac_diag* out) {
+    if (!ctx || !raws || !out || nranks < 1) return AC_EINVAL;
+    double su = 0.0, sb = 0.0, mu = 0.0, mb = 0.0, lmin = INFINITY, lmax = -INFINITY;
+    for (int r = 0; r < nranks; r++) {       // rank order: deterministic
+        const double* v = raws + 6 * r;
+        su += v[0];
+        sb += v[2];
+        mu = std::max(mu, v[1]);
+        mb = std::max(mb, v[3]);
+        lmin = std::min(lmin, v[4]);
+        lmax = std::max(lmax, v[5]);
+    }
+    const ac_grid& g = ctx->grid;
+    const double ncell = (double)g.nx * g.ny * (double)ctx->nz_global;
+    out->urms = std::sqrt(su / ncell);
+    out->umax = std::sqrt(mu);
+    out->brms = std::sqrt(sb / ncell);
+    out->bmax = std::sqrt(mb);
+    out->lnrho_min = lmin;
+    out->lnrho_max = lmax;
+    out->nonfinite = !(std::isfinite(su) && std::isfinite(sb) && std::isfinite(lmin) && std::isfinite(lmax));
+    const double hmin = std::min(g.lx / g.nx, std::min(g.ly / g.ny, g.lz / g.nz));
+    double dt = ctx->c_u * hmin / (out->umax + ctx->cs);
+    const double d = std::max(ctx->nu, ctx->eta);
+    if (d > 0.0) dt = std::min(dt, ctx->c_nu * hmin * hmin / d);
+    out->dt_cfl = dt;
+    return AC_OK;
 }
 
 int ac_state_layout(const ac_ctx* ctx, ac_layout_info* out) {
@@ -911,7 +1060,11 @@ int ac_forcing_params(double k_f, double helicity, double cs, const ac_grid* gri
 
 int ac_forcing_from_draws(const ac_ctx* ctx, double u1, double u2, double u3, double dt, double f0, ac_forcing* out) {
     if (!ctx) return AC_EINVAL;
-    return ac_forcing_params(ctx->k_f, ctx->helicity, ctx->cs, &ctx->grid, u1, u2, u3, dt, f0, out);
+    // the wave vectors count periods of the GLOBAL box: a slab knows its share of it (ac_set_slab)
+    ac_grid g = ctx->grid;
+    g.lz = ctx->grid.lz / ctx->grid.nz * ctx->nz_global;
+    g.nz = ctx->nz_global;
+    return ac_forcing_params(ctx->k_f, ctx->helicity, ctx->cs, &g, u1, u2, u3, dt, f0, out);
 }
 
 int ac_make_forcing(const ac_ctx* ctx, uint64_t seed, uint64_t step, double dt, double f0, ac_forcing* out) {

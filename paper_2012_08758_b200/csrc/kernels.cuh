@@ -65,6 +65,37 @@ __global__ void unpack_pairs_kernel(const float2* __restrict__ padded, float* __
 }
 
 // ------------------------------------------------------------------------------------------------
+// z-slab halo (NEXT-3): the 3 bottom and 3 top planes of CELLS of every field (x / y ghost zones
+// included) to and from dense buffers [7][3][my * pitch] of T.  LANES = 2: packed fp32 pairs (z, z + nz/2): the
+// bottom cells are lane 0 of planes 0..2, the top cells lane 1 of planes nzp-3..nzp-1; of a ghost plane only the
+// lane that belongs to the neighbour is written (the other lane is the slab's own cell, kept current by the
+// ghost-zone pass).
+// ------------------------------------------------------------------------------------------------
+template <typename T, int LANES>
+__global__ void halo_pack_kernel(const void* __restrict__ state, size_t field_elems, Layout L, T* __restrict__ lo,
+                                 T* __restrict__ hi) {
+    const size_t per_field = (size_t)R * L.plane;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= per_field) return;
+    const int q = blockIdx.y;
+    const T* f = (const T*)state + (size_t)q * field_elems * LANES;
+    // padded plane R + j holds cell plane j
+    lo[q * per_field + i] = f[((size_t)R * L.plane + i) * LANES];
+    hi[q * per_field + i] = f[((size_t)L.nz * L.plane + i) * LANES + (LANES - 1)];
+}
+template <typename T, int LANES>
+__global__ void halo_unpack_kernel(void* __restrict__ state, size_t field_elems, Layout L, const T* __restrict__ lo,
+                                   const T* __restrict__ hi) {
+    const size_t per_field = (size_t)R * L.plane;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= per_field) return;
+    const int q = blockIdx.y;
+    T* f = (T*)state + (size_t)q * field_elems * LANES;
+    f[i * LANES] = lo[q * per_field + i];                                                   // ghost planes below
+    f[((size_t)(L.nz + R) * L.plane + i) * LANES + (LANES - 1)] = hi[q * per_field + i];  // ghost planes above
+}
+
+// ------------------------------------------------------------------------------------------------
 // forcing tables (S7): cos/sin of k_a x_a per axis, phase folded into the z table.
 // layout: [cx(nx) sx(nx) cy(ny) sy(ny) cz(nz) sz(nz)]
 // ------------------------------------------------------------------------------------------------
@@ -118,6 +149,7 @@ struct SubstepArgs {
     Layout L;
     Coeffs<T> c;
     Physics<T> p;
+    int z_begin, z_end;   // planes updated by this launch
 };
 
 // write a new interior value and its periodic images in the ghost layers (S1 fused into S8)
@@ -145,8 +177,8 @@ __global__ void __launch_bounds__(256) substep_direct_kernel(const __grid_consta
     const Layout& L = a.L;
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
-    const int z = blockIdx.z * blockDim.z + threadIdx.z;
-    if (x >= L.nx || y >= L.ny || z >= L.nz) return;
+    const int z = a.z_begin + blockIdx.z * blockDim.z + threadIdx.z;
+    if (x >= L.nx || y >= L.ny || z >= a.z_end) return;
     const size_t c0 = L.idx(x, y, z);
     const long pitch = L.pitch;
     const long plane = (long)L.plane;

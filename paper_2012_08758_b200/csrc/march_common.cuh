@@ -63,6 +63,7 @@ struct MarchArgs {
     Layout L;            // layout in 8-byte elements; L.nz = number of (packed) planes
     int nz_full;         // planes of the caller's grid (= L.nz, or 2 L.nz for packed fp32)
     int cz;              // planes per z chunk (<= M_CZMAX)
+    int z_begin, z_end;  // planes [z_begin, z_end) are updated by this launch (the whole grid, or the inner / outer part of a slab)
     int substep;
     int has_forcing;
     int wrap_z;          // 1: write the periodic z images too (single box); 0: a slab neighbour fills the z ghost planes

@@ -98,10 +98,11 @@ __device__ __forceinline__ E m_mixxy(const E* p, const E (&cm)[3]) {
 constexpr int M_GHOST_THREADS = 256;
 constexpr int M_GHOST_ROWS_PER_TASK = M_GHOST_THREADS / (2 * R);   // interior rows whose 6 x ghosts one task copies
 template <typename E>
-__global__ void __launch_bounds__(M_GHOST_THREADS) ghost_fill_kernel(E* __restrict__ base, Layout L, int nb_rows, int na_tasks) {
+__global__ void __launch_bounds__(M_GHOST_THREADS) ghost_fill_kernel(E* __restrict__ base, Layout L, int nb_rows, int na_tasks, int first_row) {
     E* __restrict__ f = base + (size_t)blockIdx.y * L.field;
     const int tid = threadIdx.x;
-    for (int task = blockIdx.x; task < nb_rows + na_tasks; task += gridDim.x) {
+    // first_row = 2 R my skips the 6 ghost planes (a slab whose neighbours fill them)
+    for (int task = first_row + blockIdx.x; task < nb_rows + na_tasks; task += gridDim.x) {
         if (task < nb_rows) {
             // one ghost row (ghost in y or z), whole: x ghosts included
             const int row = task;
@@ -165,8 +166,8 @@ __global__ void __launch_bounds__(M_THREADS, 1)
     const int lane = tid & 31;
     const int pair = (tid >> 5) & 3;        // U warp w and A warp w + 4 serve the same 32 columns
     const int x0 = blockIdx.x * M_TX, y0 = blockIdx.y * M_TY;
-    const int zs = blockIdx.z * a.cz;
-    const int ze = min(zs + a.cz, L.nz);
+    const int zs = a.z_begin + blockIdx.z * a.cz;
+    const int ze = min(zs + a.cz, a.z_end);
     const int niter = ze - zs + 2 * R;      // planes zs-3 .. ze+2
     const int x = x0 + tx, y = y0 + ty;
     const bool valid = (x < L.nx) && (y < L.ny);

@@ -314,8 +314,8 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
     const int ty0 = 2 * (2 * wp + (lane >> 4));
     const int col0 = ty0 * Q_TX + tx;          // cell c of the pair: col0 + c * Q_TX
     const int x0 = blockIdx.x * Q_TX, y0 = blockIdx.y * Q_TY;
-    const int zs = blockIdx.z * a.cz;
-    const int ze = min(zs + a.cz, L.nz);
+    const int zs = a.z_begin + blockIdx.z * a.cz;
+    const int ze = min(zs + a.cz, a.z_end);
     const int niter = ze - zs + 2 * R;      // planes zs-3 .. ze+2
     const int x = x0 + tx, y = y0 + ty0;
     const bool with_prev = a.substep != 0;

@@ -1,15 +1,14 @@
-"""z-slab decomposition of the box over several ranks: host-side orchestration only.
+"""z-slab decomposition of the box over several ranks: host-side orchestration only, no
+arithmetic of the method (the phase shift of the forcing, the halo lanes of packed fp32 pairs and the combination of
+the diagnostics all live behind the C ABI: ac_set_slab, ac_halo_pack / ac_halo_unpack, ac_diag_combine).
 
-Every rank owns nz / p planes and runs the ordinary single-GPU context on them (its ac_grid has nz = nz_local and
-lz = L_z / p).  After every substep the 3 ghost planes per side of all 7 fields are replaced by the neighbour ranks'
-boundary planes; in the padded device layout those are contiguous blocks, so the exchange is plain copies: peer
-sends/receives through torch.distributed (one process per GPU, NCCL) or, for several slabs held by one process on one
-GPU (the test set-up), device-to-device copies.  No kernel waits on another rank.  The reductions are combined from
-the ranks' raw sums.  Only layouts without packed fp32 pairs can be exchanged this way: fp64, or fp32 with the direct
-kernel variant.
+Every rank owns nz / p planes and runs the ordinary context on them.  A substep follows the paper's schedule
+(Fig. 3): the halo of the current state travels on a second stream (pack -> send / receive -> unpack)
+WHILE the inner planes are updated on the compute stream; the 3 + 3 boundary planes follow once the halo has landed.
+Transport: torch.distributed point-to-point operations on the dense halo buffers (NCCL between GPUs; gloo with host
+staging for the multi-process test on one GPU), or device-to-device copies for several slabs held by one process (the
+one-GPU emulation).  No kernel waits on another rank.
 """
-import math
-
 import numpy as np
 
 from . import binding
@@ -22,124 +21,173 @@ def local_lengths(lengths, world):
     return (lx, ly, lz / world)
 
 
-def rank_forcing(forcing, z0):
-    """The forcing of Eq. 4 seen from a slab whose first plane sits at z0: phase + k_z z0."""
-    if forcing is None:
-        return None
-    if isinstance(forcing, binding.AcForcing):
-        forcing = (tuple(forcing.k), forcing.phase, tuple(forcing.re), tuple(forcing.im))
-    k, phase, re, im = forcing
-    return (k, phase + k[2] * z0, re, im)
+class _HostStream:
+    """Stand-in for a CUDA stream / event when a context lives on the host (the CPU tests of the schedule drive this
+    module with a numpy stand-in for binding.Context): every call completes before it returns."""
+    cuda_stream = 0
+
+    def wait_event(self, ev):
+        pass
+
+    def wait_stream(self, st):
+        pass
+
+    def synchronize(self):
+        pass
+
+    def record(self, st=None):
+        pass
 
 
 class Slab:
-    """One rank's context plus views of its halo planes."""
+    """One rank's context, its halo buffers and its two streams."""
 
-    def __init__(self, global_shape, lengths, rank, world, dtype=binding.AC_F64, **kw):
+    def __init__(self, global_shape, lengths, rank, world, dtype=binding.AC_F64, variant=0, context_factory=None, **kw):
         import torch
         nz, ny, nx = global_shape
         if nz % world != 0 or nz // world < 8:
             raise binding.AcError("nz must split into slabs of at least 8 planes")
         self.rank, self.world, self.nzl = rank, world, nz // world
-        self.z0 = rank * self.nzl * (lengths[2] / nz)
-        self.ctx = binding.Context((self.nzl, ny, nx), local_lengths(lengths, world), dtype, **kw)
-        if dtype == binding.AC_F32:
-            self.ctx.ac_set_variant(1)              # plain float layout: ghost planes are plain planes
-        info = self.ctx.ac_state_layout()
-        if info.packed_pairs:
-            raise binding.AcError("packed fp32 pairs cannot be exchanged plane-wise")
-        self.info = info
-        self.tdtype = torch.float64 if info.elem_bytes == 8 else torch.float32
-        self._flat = self.ctx.workspace.view(torch.uint8)
+        make = context_factory or binding.Context
+        self.ctx = make((self.nzl, ny, nx), local_lengths(lengths, world), dtype, **kw)
+        self.ctx.ac_set_variant(variant)
+        self.ctx.ac_set_slab(rank * self.nzl, nz)
+        dev = self.ctx.device
+        nb = self.ctx.ac_halo_bytes()
+        self.send_lo, self.send_hi, self.recv_lo, self.recv_hi = (torch.empty(nb, dtype=torch.uint8, device=dev)
+                                                                  for _ in range(4))
+        if torch.device(dev).type == "cuda":
+            with torch.cuda.device(dev):
+                self.comm = torch.cuda.Stream(device=dev)
+            self.state_ready = torch.cuda.Event()
+            self.halo_ready = torch.cuda.Event()
+        else:
+            self.comm = self.state_ready = self.halo_ready = _HostStream()
+        self.halo_valid = False           # do the z ghost planes of the current state hold the neighbours' planes?
 
-    def _planes(self, q, first):
-        """torch view of 3 padded planes of field q of the current state, starting at padded plane `first`."""
-        import torch
-        base = self.ctx.ac_field_device_ptr(q) - self._flat.data_ptr()
-        eb = self.info.elem_bytes
-        start = base + first * self.info.plane_elems * eb
-        n = R * self.info.plane_elems
-        return self._flat[start:start + n * eb].view(self.tdtype)
+    # the three phases of an exchange, all on the communication stream
+    def pack(self):
+        self.state_ready.record(self.ctx.stream)
+        self.comm.wait_event(self.state_ready)
+        self.ctx.ac_halo_pack(self.send_lo, self.send_hi, self.comm)
 
-    def halo(self):
-        """(send_up, send_dn, recv_lo, recv_hi): lists of 7 views each."""
-        nzl = self.nzl
-        return ([self._planes(q, nzl) for q in range(7)], [self._planes(q, R) for q in range(7)],
-                [self._planes(q, 0) for q in range(7)], [self._planes(q, nzl + R) for q in range(7)])
+    def unpack(self):
+        self.ctx.ac_halo_unpack(self.recv_lo, self.recv_hi, self.comm)
+        self.halo_ready.record(self.comm)
+        self.halo_valid = True
+
+    def wait_halo(self):
+        self.ctx.stream.wait_event(self.halo_ready)
 
 
-def exchange_in_process(slabs):
-    """All slabs live in this process on one device: ghost planes <- neighbours' boundary planes."""
+def transfer_in_process(slabs):
+    """All slabs live in this process on one device: neighbour buffers by device-to-device copies."""
+    import torch
     p = len(slabs)
-    halos = [s.halo() for s in slabs]
-    for r in range(p):
-        up, dn = halos[(r - 1) % p][0], halos[(r + 1) % p][1]
-        for q in range(7):
-            halos[r][2][q].copy_(up[q])
-            halos[r][3][q].copy_(dn[q])
+    cuda = slabs[0].send_lo.is_cuda
+    for r, s in enumerate(slabs):
+        below, above = slabs[(r - 1) % p], slabs[(r + 1) % p]
+        s.comm.wait_stream(below.comm)                           # their packs
+        s.comm.wait_stream(above.comm)
+        with (torch.cuda.stream(s.comm) if cuda else _Null()):
+            s.recv_lo.copy_(below.send_hi, non_blocking=True)    # the top planes of the slab below
+            s.recv_hi.copy_(above.send_lo, non_blocking=True)    # the bottom planes of the slab above
+    for r, s in enumerate(slabs):                                # nobody repacks a buffer a neighbour still reads
+        s.comm.wait_stream(slabs[(r - 1) % p].comm)
+        s.comm.wait_stream(slabs[(r + 1) % p].comm)
 
 
-def ring_exchange(send_up, send_dn, recv_lo, recv_hi, dist, rank, world):
-    """One process per rank: 2 sends and 2 receives of the 7 fields' planes, staged in one buffer each.
-    send_up goes to rank + 1 (its lower ghost planes), send_dn to rank - 1 (its upper ghost planes)."""
+class _Null:
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        return False
+
+
+def ring_transfer(send_lo, send_hi, recv_lo, recv_hi, dist, rank, world, stream=None):
+    """One process per rank: send_hi goes to rank + 1 (its recv_lo), send_lo to rank - 1 (its recv_hi); 2 sends and
+    2 receives of whole halo buffers.  NCCL: enqueued on `stream`, nothing blocks the host.  gloo: device buffers
+    are staged through the host (test set-up: several ranks sharing one GPU); host buffers go as they are."""
     import torch
     up, dn = (rank + 1) % world, (rank - 1) % world
-    s_up, s_dn = torch.stack(list(send_up)), torch.stack(list(send_dn))
-    if s_up.is_cuda and dist.get_backend() != "nccl":
-        # gloo moves host memory: stage through the CPU (test set-up: several ranks sharing one GPU)
-        s_up, s_dn = s_up.cpu(), s_dn.cpu()
-    r_lo, r_hi = torch.empty_like(s_up), torch.empty_like(s_dn)
-    ops = [dist.P2POp(dist.isend, s_up, up), dist.P2POp(dist.isend, s_dn, dn),
+    if dist.get_backend() == "nccl":
+        with torch.cuda.stream(stream):
+            ops = [dist.P2POp(dist.isend, send_hi, up), dist.P2POp(dist.isend, send_lo, dn),
+                   dist.P2POp(dist.irecv, recv_lo, dn), dist.P2POp(dist.irecv, recv_hi, up)]
+            for req in dist.batch_isend_irecv(ops):
+                req.wait()                                      # stream-ordered for NCCL
+        return
+    if send_hi.is_cuda:
+        stream.synchronize()
+        s_hi, s_lo = send_hi.cpu(), send_lo.cpu()
+        r_lo, r_hi = torch.empty_like(s_hi), torch.empty_like(s_lo)
+    else:
+        s_hi, s_lo, r_lo, r_hi = send_hi, send_lo, recv_lo, recv_hi
+    ops = [dist.P2POp(dist.isend, s_hi, up), dist.P2POp(dist.isend, s_lo, dn),
            dist.P2POp(dist.irecv, r_lo, dn), dist.P2POp(dist.irecv, r_hi, up)]
     for req in dist.batch_isend_irecv(ops):
         req.wait()
-    for q in range(len(recv_lo)):
-        recv_lo[q].copy_(r_lo[q])
-        recv_hi[q].copy_(r_hi[q])
+    if send_hi.is_cuda:
+        with torch.cuda.stream(stream):
+            recv_lo.copy_(r_lo, non_blocking=False)
+            recv_hi.copy_(r_hi, non_blocking=False)
 
 
-def combine_raw(raws, ncell_global, h, nu, eta, cs, c_u=0.4, c_nu=0.25):
-    """Diagnostics of the whole box from the ranks' ac_reduce_raw tuples (G15, G18)."""
-    su = sum(r[0] for r in raws)
-    sb = sum(r[2] for r in raws)
-    mu = max(r[1] for r in raws)
-    mb = max(r[3] for r in raws)
-    umax = math.sqrt(mu)
-    dt = c_u * h / (umax + cs)
-    if max(nu, eta) > 0:
-        dt = min(dt, c_nu * h * h / max(nu, eta))
-    return {"urms": math.sqrt(su / ncell_global), "umax": umax, "brms": math.sqrt(sb / ncell_global),
-            "bmax": math.sqrt(mb), "lnrho_min": min(r[4] for r in raws), "lnrho_max": max(r[5] for r in raws),
-            "dt_cfl": dt}
+def transfer_distributed(slab, dist):
+    ring_transfer(slab.send_lo, slab.send_hi, slab.recv_lo, slab.recv_hi, dist, slab.rank, slab.world, slab.comm)
 
 
 class SlabGroupInProcess:
     """p slabs of one box driven by one process on one GPU: the reference behaviour of the decomposition."""
 
-    def __init__(self, global_shape, lengths, world, dtype=binding.AC_F64, **kw):
-        self.shape, self.lengths, self.kw = tuple(global_shape), tuple(lengths), kw
-        self.slabs = [Slab(global_shape, lengths, r, world, dtype, **kw) for r in range(world)]
+    def __init__(self, global_shape, lengths, world, dtype=binding.AC_F64, variant=0, overlap=True, context_factory=None,
+                 **kw):
+        self.shape, self.lengths, self.kw, self.overlap = tuple(global_shape), tuple(lengths), kw, overlap
+        self.slabs = [Slab(global_shape, lengths, r, world, dtype, variant, context_factory, **kw) for r in range(world)]
+
+    def exchange(self):
+        for s in self.slabs:
+            s.pack()
+        transfer_in_process(self.slabs)
+        for s in self.slabs:
+            s.unpack()
 
     def load_state(self, state):
         nzl = self.slabs[0].nzl
         for s in self.slabs:
             s.ctx.ac_load_state(np.ascontiguousarray(state[:, s.rank * nzl:(s.rank + 1) * nzl]))
-        exchange_in_process(self.slabs)
+            s.halo_valid = False
 
     def step(self, dt, forcing=None):
+        """forcing: of the GLOBAL box (every slab shifts the phase itself)."""
         for sub in range(3):
             for s in self.slabs:
-                s.ctx.ac_substep(sub, dt, rank_forcing(forcing, s.z0))
-            exchange_in_process(self.slabs)
+                s.pack()                                      # communication stream, after the previous substep
+                if self.overlap:
+                    s.ctx.ac_substep_part(sub, dt, forcing, binding.AC_PART_INNER)    # runs beside the exchange
+            transfer_in_process(self.slabs)
+            for s in self.slabs:
+                s.unpack()
+                s.wait_halo()
+                if self.overlap:
+                    s.ctx.ac_substep_part(sub, dt, forcing, binding.AC_PART_OUTER)
+                else:
+                    s.ctx.ac_substep(sub, dt, forcing)
+                s.halo_valid = False
+
+    def make_forcing(self, seed, step, dt, f0):
+        return self.slabs[0].ctx.ac_make_forcing(seed, step, dt, f0)
 
     def store_state(self):
         return np.concatenate([s.ctx.ac_store_state() for s in self.slabs], axis=1)
 
     def reduce(self):
-        nz, ny, nx = self.shape
-        h = min(self.lengths[0] / nx, self.lengths[1] / ny, self.lengths[2] / nz)
-        return combine_raw([s.ctx.ac_reduce_raw() for s in self.slabs], nz * ny * nx, h, self.kw.get("nu", 0.0),
-                           self.kw.get("eta", 0.0), self.kw.get("cs", 1.0))
+        if not all(s.halo_valid for s in self.slabs):
+            self.exchange()
+        for s in self.slabs:
+            s.wait_halo()
+        return self.slabs[0].ctx.ac_diag_combine([s.ctx.ac_reduce_raw() for s in self.slabs])
 
     def free(self):
         for s in self.slabs:
@@ -149,22 +197,26 @@ class SlabGroupInProcess:
 class SlabRank:
     """One process per rank (torchrun): this rank's slab of the box, exchanged through torch.distributed."""
 
-    def __init__(self, global_shape, lengths, dist, dtype=binding.AC_F64, device="cuda:0", **kw):
+    def __init__(self, global_shape, lengths, dist, dtype=binding.AC_F64, device="cuda:0", variant=0, overlap=True,
+                 context_factory=None, **kw):
         self.dist, self.rank, self.world = dist, dist.get_rank(), dist.get_world_size()
-        self.shape, self.lengths, self.kw = tuple(global_shape), tuple(lengths), kw
-        self.slab = Slab(global_shape, lengths, self.rank, self.world, dtype, device=device, **kw)
+        self.shape, self.lengths, self.kw, self.overlap = tuple(global_shape), tuple(lengths), kw, overlap
+        self.slab = Slab(global_shape, lengths, self.rank, self.world, dtype, variant, context_factory, device=device, **kw)
 
     def forcing_from_draws(self, u1, u2, u3, dt, f0):
-        """Eq. 4-6 for the GLOBAL box (the slab's own context would take its shorter l_z for the box length)."""
-        f = binding.ac_forcing_params(self.kw.get("k_f", 3.0), self.kw.get("helicity", 0.0), self.kw.get("cs", 1.0),
-                                      self.shape, self.lengths, u1, u2, u3, dt, f0)
-        return (tuple(f.k), f.phase, tuple(f.re), tuple(f.im))
+        """Eq. 4-6 for the GLOBAL box (a slab context knows the global box, ac_set_slab)."""
+        return self.slab.ctx.ac_forcing_from_draws(u1, u2, u3, dt, f0)
+
+    def transfer(self):
+        if self.world > 1:
+            transfer_distributed(self.slab, self.dist)
+        else:
+            transfer_in_process([self.slab])                  # a single rank is its own neighbour
 
     def exchange(self):
-        if self.world == 1:
-            return                                  # the rank's own periodic images are already right
-        self.slab.ctx.synchronize()
-        ring_exchange(*self.slab.halo(), self.dist, self.rank, self.world)
+        self.slab.pack()
+        self.transfer()
+        self.slab.unpack()
 
     def load_state(self, state):
         """state: the GLOBAL (7, nz, ny, nx) array (every rank generates the same seeded input) or this rank's slab."""
@@ -172,25 +224,34 @@ class SlabRank:
         if state.shape[1] != nzl:
             state = state[:, self.rank * nzl:(self.rank + 1) * nzl]
         self.slab.ctx.ac_load_state(np.ascontiguousarray(state))
-        self.exchange()
+        self.slab.halo_valid = False
 
     def step(self, dt, forcing=None):
-        f = rank_forcing(forcing, self.slab.z0)
+        s = self.slab
         for sub in range(3):
-            self.slab.ctx.ac_substep(sub, dt, f)
-            self.exchange()
+            s.pack()                                          # communication stream, after the previous substep
+            if self.overlap:
+                s.ctx.ac_substep_part(sub, dt, forcing, binding.AC_PART_INNER)        # runs beside the exchange
+            self.transfer()
+            s.unpack()
+            s.wait_halo()
+            if self.overlap:
+                s.ctx.ac_substep_part(sub, dt, forcing, binding.AC_PART_OUTER)
+            else:
+                s.ctx.ac_substep(sub, dt, forcing)
+            s.halo_valid = False
 
     def reduce(self):
         import torch
+        if not self.slab.halo_valid:
+            self.exchange()
+        self.slab.wait_halo()
         raw = torch.tensor(self.slab.ctx.ac_reduce_raw(), dtype=torch.float64)
         if self.world > 1:
-            allr = [torch.empty_like(raw) for _ in range(self.world)]
-            dev = raw.cuda() if self.dist.get_backend() == "nccl" else raw
+            dev = raw.to(self.slab.ctx.device) if self.dist.get_backend() == "nccl" else raw
             allr = [torch.empty_like(dev) for _ in range(self.world)]
             self.dist.all_gather(allr, dev)
             raws = [tuple(t.cpu().tolist()) for t in allr]
         else:
             raws = [tuple(raw.tolist())]
-        nz, ny, nx = self.shape
-        h = min(self.lengths[0] / nx, self.lengths[1] / ny, self.lengths[2] / nz)
-        return combine_raw(raws, nz * ny * nx, h, self.kw.get("nu", 0.0), self.kw.get("eta", 0.0), self.kw.get("cs", 1.0))
+        return self.slab.ctx.ac_diag_combine(raws)

@@ -13,18 +13,21 @@ import helpers
 pytestmark = pytest.mark.gpu
 
 
+@pytest.mark.parametrize("overlap", [True, False])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("dtype", [binding.AC_F64, binding.AC_F32])
 @pytest.mark.parametrize("world", [2, 3])
-def test_slabs_equal_single_context(world, dtype):
+def test_slabs_equal_single_context(world, dtype, variant, overlap):
+    """Every kernel variant, both precisions (fp32 variants 0 and 2 on the packed-pair layout, whose halo lanes
+    ac_halo_pack / ac_halo_unpack pick), with the inner / outer split of the paper's schedule and without it."""
     shape = (48, 24, 32)
     lengths = (2 * math.pi, 1.5 * math.pi, 3.0 * math.pi)
     npdt = np.float64 if dtype == binding.AC_F64 else np.float32
     state = inputs.smooth_strong_state(shape, 41).astype(npdt)
     kw = dict(nu=5e-3, eta=4e-3, cs=1.0, k_f=3, helicity=1.0)
     one = binding.Context(shape, lengths, dtype, **kw)
-    if dtype == binding.AC_F32:
-        one.ac_set_variant(1)                      # same kernel as the slabs use in fp32
-    grp = slab.SlabGroupInProcess(shape, lengths, world, dtype, **kw)
+    one.ac_set_variant(variant)
+    grp = slab.SlabGroupInProcess(shape, lengths, world, dtype, variant=variant, overlap=overlap, **kw)
     one.ac_load_state(state)
     grp.load_state(state)
     dt = 2e-3
@@ -64,8 +67,22 @@ def test_three_substeps_equal_one_step():
     assert np.array_equal(a.ac_store_state(), b.ac_store_state())
     with pytest.raises(binding.AcError):
         b.ac_substep(3, 1e-3, f)
+    # and so do inner + outer parts (an ordinary box: the ghost planes are the box's own periodic images)
+    c = binding.Context(shape, nu=1e-2, eta=1e-2)
+    c.ac_load_state(state)
+    for s in range(3):
+        with pytest.raises(binding.AcError):
+            c.ac_substep_part(s, 1e-3, f, binding.AC_PART_OUTER)          # outer before inner
+        c.ac_substep_part(s, 1e-3, f, binding.AC_PART_INNER)
+        with pytest.raises(binding.AcError):
+            c.ac_substep_part(s, 1e-3, f, binding.AC_PART_INNER)          # twice
+        with pytest.raises(binding.AcError):
+            c.ac_substep(s, 1e-3, f)
+        c.ac_substep_part(s, 1e-3, f, binding.AC_PART_OUTER)
+    assert np.array_equal(a.ac_store_state(), c.ac_store_state())
     a.ac_free()
     b.ac_free()
+    c.ac_free()
 
 
 def test_slab_ranks_as_processes(tmp_path):
