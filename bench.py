@@ -8,8 +8,10 @@ whole hot path over one synthetic box.  Default workload: BASELINE config 4 (512
 helical forcing k_f = 3, f0 = 0.02, seeded solenoidal u of rms 0.1, weak Gaussian A, fixed CFL dt).
 Prints ONE JSON line (see DESIGN.md "Measurement" for every key).
 
-N > 1: the path does not shard yet (one GPU only): each rank advances an
-independent replica of the box, value = N boxes' cells / max-over-ranks time ("replicas only").
+N > 1 (torchrun, or `--gpus N` alone: the script then starts its N ranks itself): the ranks share ONE box as z slabs
+with a halo exchange per substep overlapped with the inner-domain update:
+strong scaling at the workload's size; `--weak` gives every rank a full n^2 x n slab (the paper's two protocols,
+PAPER.md:533); `--replicas` runs N independent boxes instead.
 """
 import argparse
 import json
@@ -119,7 +121,7 @@ def time_oracle(n_sample, cfg, steps, warmup=0):
         st.step(dt, f)
         if s >= warmup:
             times.append(time.perf_counter() - t0)
-    return n_sample ** 3 / float(np.mean(times)), float(np.mean(times)), mhd_c.max_threads()
+    return n_sample ** 3 / float(np.median(times)), float(np.median(times)), mhd_c.max_threads()
 
 
 def max_over_ranks(ms, dist, device):
@@ -292,20 +294,28 @@ def run_ours(args):
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        n_s = min(n, args.ref_sample)
-        v, sec, cores = time_oracle(n_s, cfg, 1)
-        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "ns_per_cell_step": 1e9 / v,
-               "sample": "1 RK3 step of the C oracle (fp64, OpenMP) on a %d^3 box of the same recipe; %.1f s" % (n_s, sec)}
-        # the same oracle on one thread, on a 64^3 box to keep the run short
+        # the oracle as it stands on 128^3 and 256^3 boxes of the same recipe, all host cores, one
+        # untimed warm-up step (thread start-up, first-touch page faults) and the median of the timed ones; and on one
+        # thread (64^3 to keep the run short)
         from oracle import mhd_c
+        n_s = min(n, args.ref_sample)
+        v, sec, cores = time_oracle(n_s, cfg, 3, 1)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "ns_per_cell_step": 1e9 / v,
+               "sample": "C oracle (fp64, OpenMP) on a %d^3 box of the same recipe: 1 warm-up + 3 timed RK3 steps, "
+                         "median %.2f s per step" % (n_s, sec)}
+        if n >= 256 and not args.quick_cpu:
+            v2, sec2, _ = time_oracle(256, cfg, 2, 1)
+            cpu["box_256"] = {"value": v2, "unit": UNIT, "ns_per_cell_step": 1e9 / v2,
+                              "sample": "256^3 box: 1 warm-up + 2 timed steps, median %.2f s per step" % sec2}
         nthreads = mhd_c.max_threads()
         mhd_c.set_threads(1)
         try:
-            v1, sec1, _ = time_oracle(min(n_s, 64), cfg, 1)
+            v1, sec1, _ = time_oracle(min(n_s, 64), cfg, 3, 1)
         finally:
             mhd_c.set_threads(nthreads)
         cpu["one_thread"] = {"value": v1, "unit": UNIT, "ns_per_cell_step": 1e9 / v1,
-                             "sample": "1 step on a %d^3 box, 1 thread; %.1f s" % (min(n_s, 64), sec1)}
+                             "sample": "%d^3 box, 1 thread: 1 warm-up + 3 timed steps, median %.2f s per step"
+                                       % (min(n_s, 64), sec1)}
 
     if rank == 0:
         line = {
@@ -334,8 +344,9 @@ def run_ours(args):
 
 
 def run_slab(args):
-    """N ranks share ONE box as z slabs: strong scaling, halo planes exchanged after every
-    substep through torch.distributed (NCCL).  fp64 only.  Not the default for --gpus N (that is "replicas only")."""
+    """N ranks share ONE box as z slabs: the halo of the current state
+    travels on a second stream while the inner planes are updated, the boundary planes follow (slab.SlabRank).
+    Strong scaling (one n^3 box over N ranks) or, with --weak, n^2 x n per rank."""
     import torch
     import torch.distributed as dist
     from paper_2012_08758_b200 import binding, inputs, slab
@@ -351,56 +362,96 @@ def run_slab(args):
     n = args.n
     cfg = workload(n)
     nu = cfg["nu"]
-    rk = slab.SlabRank((n, n, n), TWO_PI3, dist, binding.AC_F64, device="cuda:%d" % local_rank, nu=nu, eta=nu, cs=1.0,
-                       k_f=3.0, helicity=cfg["sigma"])
-    nzl = rk.slab.nzl
-    local = np.empty((7, nzl, n, n))
-    for q, field in enumerate(inputs.solenoidal_state_fields(n, cfg["seed"])):
-        local[q] = field[rank * nzl:(rank + 1) * nzl]
-    del field
-    rk.load_state(local)
-    dt = rk.reduce()["dt_cfl"]
-    draws = [inputs.counter_uniforms(cfg["seed"] + 7, s) for s in range(args.warmup + args.steps)]
-    forcings = [rk.forcing_from_draws(*u, dt, 0.02) for u in draws]
-    for s in range(args.warmup):
-        rk.step(dt, forcings[s])
-    torch.cuda.synchronize()
-    dist.barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    l0 = rk.slab.ctx.ac_launch_count()
-    e0.record(rk.slab.ctx.stream)
-    for s in range(args.steps):
-        rk.step(dt, forcings[args.warmup + s])
-    e1.record(rk.slab.ctx.stream)
-    torch.cuda.synchronize()
-    dist.barrier()
-    clocks = sampler.stop()
-    total_ms = max_over_ranks(e0.elapsed_time(e1), dist if world > 1 else None, "cuda")
-    launches = rk.slab.ctx.ac_launch_count() - l0
-    diag = rk.reduce()
-    ms_per_step = total_ms / args.steps
-    value = n ** 3 / (ms_per_step * 1e-3)
+    nz_global = n * world if args.weak else n
+    lengths = (2 * math.pi, 2 * math.pi, 2 * math.pi * nz_global / n)
     peak, peak_src = measured_peak()
-    alg = WORDS_PER_CELL_STEP / 3.0 * 8 * n ** 3 / world        # per rank and launch
-    achieved = alg / (ms_per_step / 3.0 * 1e-3) / 1e9
-    halo_bytes = 2 * 7 * 3 * rk.slab.info.plane_elems * 8
+
+    def bench_dtype(dtype_name):
+        dtype = binding.AC_F64 if dtype_name == "f64" else binding.AC_F32
+        npdt = np.float64 if dtype_name == "f64" else np.float32
+        es = 8 if dtype_name == "f64" else 4
+        rk = slab.SlabRank((nz_global, n, n), lengths, dist, dtype, device="cuda:%d" % local_rank, variant=args.variant,
+                           overlap=not args.no_overlap, nu=nu, eta=nu, cs=1.0, k_f=3.0, helicity=cfg["sigma"])
+        nzl = rk.slab.nzl
+        local = np.empty((7, nzl, n, n), dtype=npdt)
+        for q, field in enumerate(inputs.solenoidal_state_fields(n, cfg["seed"])):
+            # strong: this rank's planes of the one box; weak: every rank holds planes of the same seeded n^3 box
+            local[q] = field[(rank * nzl) % n:(rank * nzl) % n + nzl]
+        del field
+        rk.load_state(local)
+        dt = rk.reduce()["dt_cfl"]
+        draws = [inputs.counter_uniforms(cfg["seed"] + 7, s) for s in range(args.warmup + args.steps)]
+        forcings = [rk.forcing_from_draws(*u, dt, 0.02) for u in draws]
+        for s in range(args.warmup):
+            rk.step(dt, forcings[s])
+        torch.cuda.synchronize()
+        dist.barrier()
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = rk.slab.ctx.ac_launch_count()
+        e0.record(rk.slab.ctx.stream)
+        for s in range(args.steps):
+            rk.step(dt, forcings[args.warmup + s])
+        e1.record(rk.slab.ctx.stream)
+        torch.cuda.synchronize()
+        dist.barrier()
+        clocks = sampler.stop()
+        total_ms = max_over_ranks(e0.elapsed_time(e1), dist if world > 1 else None, "cuda")
+        launches = rk.slab.ctx.ac_launch_count() - l0
+        diag = rk.reduce()
+        ms_per_step = total_ms / args.steps
+        cells = n * n * nz_global
+        alg = WORDS_PER_CELL_STEP / 3.0 * es * cells / world        # per rank and launch
+        achieved = alg / (ms_per_step / 3.0 * 1e-3) / 1e9
+        res = {"value": cells / (ms_per_step * 1e-3), "ms_per_step": ms_per_step, "dt": dt, "launches": launches,
+               "clocks": clocks, "diag": {k: diag[k] for k in ("urms", "brms", "nonfinite")},
+               "halo_bytes": 2 * rk.slab.ctx.ac_halo_bytes(),
+               "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                            "traffic": committed_traffic(dtype_name), "peak_source": peak_src,
+                            "kernel": "substep (per rank; inner + outer launches, halo pack / unpack and ghost kernels "
+                                      "charged to it)",
+                            "algorithmic_bytes_per_launch": alg}}
+        rk.slab.ctx.ac_free()
+        del rk, local
+        torch.cuda.empty_cache()
+        return res
+
+    main_res = bench_dtype(args.dtype)
+    other_name = "f32" if args.dtype == "f64" else "f64"
+    other = bench_dtype(other_name) if not args.single_dtype else None
     if rank == 0:
-        print(json.dumps({
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg["name"], "grid": [n, n, n], "nu": nu, "eta": nu, "helicity": cfg["sigma"], "k_f": 3,
-                       "f0": 0.02, "dt": dt, "parallelism": "z slabs x%d, halo exchange per substep" % world,
+        line = {
+            "metric": METRIC, "value": main_res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": main_res["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak" if args.weak else "strong", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+            "config": {"workload": cfg["name"] + (" x%d along z (weak)" % world if args.weak else ""),
+                       "grid": [n, n, nz_global], "nu": nu, "eta": nu, "helicity": cfg["sigma"], "k_f": 3, "f0": 0.02,
+                       "dt": main_res["dt"], "variant": args.variant,
+                       "parallelism": "z slabs x%d; halo of 3 planes per side and field per substep, %s" % (
+                           world, "exchanged on a second stream beside the inner-domain update (PAPER.md:141-158)"
+                           if not args.no_overlap else "exchanged before the substep (no overlap)"),
                        "l2": "state far larger than L2; no flush needed",
-                       "halo_bytes_per_rank_per_substep": halo_bytes},
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": committed_traffic("f64"), "peak_source": peak_src,
-                         "kernel": "substep (per rank; halo exchange and ghost kernels charged to it)"},
-            "cpu_baseline": None, "e2e": None, "gpu_launches": launches, "clocks": clocks,
-            "diag": {k: diag[k] for k in ("urms", "brms")}}))
+                       "halo_bytes_per_rank_per_substep": main_res["halo_bytes"]},
+            "roofline": main_res["roofline"], "cpu_baseline": None, "e2e": None, "gpu_launches": main_res["launches"],
+            "clocks": main_res["clocks"], "diag": main_res["diag"]}
+        if other is not None:
+            line["also"] = {"dtype": other_name, "value": other["value"], "ms_per_step": other["ms_per_step"],
+                            "roofline": other["roofline"], "clocks": other["clocks"], "gpu_launches": other["launches"]}
+        print(json.dumps(line))
     dist.destroy_process_group()
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without torchrun: start the N ranks (one per GPU) the way the driver would."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
 
 
 def main():
@@ -414,16 +465,23 @@ def main():
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--single-dtype", action="store_true", help="skip the second precision")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--quick-cpu", action="store_true", help="cpu_baseline without the 256^3 box")
     ap.add_argument("--ref-sample", type=int, default=128, help="box size of the bounded oracle sample")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--slab", action="store_true",
-                    help="N ranks share one box as z slabs with a halo exchange per substep (strong scaling, fp64)")
+                    help="run through slab.SlabRank even on one GPU (N > 1 always does unless --replicas)")
+    ap.add_argument("--replicas", action="store_true", help="N > 1: N independent boxes instead of one box in z slabs")
+    ap.add_argument("--weak", action="store_true", help="slab run with n^2 x n cells per rank (weak scaling, PAPER.md:533)")
+    ap.add_argument("--no-overlap", action="store_true", help="slab run: exchange before the substep instead of beside it")
     ap.add_argument("--paper-protocol", action="store_true",
                     help="the paper's benchmark set-up (PAPER.md:533): all fields U[0,1), no forcing, dt = 1.19209e-7")
     args = ap.parse_args()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         run_reference(args)
-    elif args.slab:
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args)
+    elif args.slab or args.weak or (world > 1 and not args.replicas):
         run_slab(args)
     else:
         run_ours(args)

