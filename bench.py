@@ -248,12 +248,17 @@ def run_ours(args):
             "s9_reduce": {"ms": red_ms, "algorithmic_bytes": 7 * es * n ** 3,
                           "achieved": 7 * es * n ** 3 / (red_ms * 1e-3) / 1e9, "unit": "GB/s",
                           "frac": 7 * es * n ** 3 / (red_ms * 1e-3) / 1e9 / measured_peak()[0],
-                          "what": "ac_reduce (stage-1 + stage-2 kernels + 48-byte D2H), median of 5"},
+                          "words_per_cell": 7,
+                          "what": "ac_reduce (stage-1 + stage-2 kernels + 48-byte D2H), median of 5; algorithmic bytes "
+                                  "count 7 words per cell (u, A and ln rho: the kernel also reduces min / max ln rho and "
+                                  "checks it for non-finite values); SURVEY.md 8(d)'s 6-word count gives 6/7 of frac"},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": committed_traffic(dtype_name), "peak_source": peak_src,
                          "kernel": "substep (avg of the 3 launches of a step)",
                          "note": "reported against HBM as BASELINE.json's metric asks; the kernel itself is limited by "
-                                 "the shared-memory data pipe (81 % of peak, profiles/r01d_march.md) and the 1000 W power cap",
+                                 "issue slots and the FP64 (fp32: packed FMA) pipe at two worker warps per scheduler "
+                                 "(57 % / 56 % busy, LSU pipe 66 %: profiles/r02_pair.md) and by the 1000 W power cap; "
+                                 "the ghost-zone kernel's time (3.4 %) is charged to the substep kernel",
                          "algorithmic_bytes_per_launch": alg_bytes_launch},
         }
         if do_e2e:

@@ -234,6 +234,9 @@ def test_sampled_parity_at_baseline_sizes(dtype, n):
     rng = np.random.default_rng(n)
     cells = [(0, 0, 0), (n - 1, n - 1, n - 1), (0, n - 1, 5), (n // 2, 0, n - 2), (3, n - 3, n // 2)]
     cells += [tuple(int(v) for v in rng.integers(0, n, 3)) for _ in range(7)]
+    # the seams: last / first column and row of a 16 x 16 tile (and of the 16 x 8 tiles of variant 2), both cells of
+    # a y-pair, the planes where the packed fp32 halves meet (z = n/2 - 1, n/2) and the first planes of the march
+    cells += [(n // 2 - 1, 15, 15), (n // 2, 16, 16), (2, 31, 32), (n - 4, 8, 47), (3, 7, 16), (n // 2 + 2, 240, 255)]
     s_u = float(np.abs(state[1:4]).max())
     s_a = float(np.abs(state[4:7]).max())
     scale = np.array([s_u, s_u, s_u, s_u, s_a, s_a, s_a])

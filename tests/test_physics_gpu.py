@@ -76,7 +76,11 @@ def test_growth_rate_of_brms_matches_tables_1_and_2(sigma, table, dtype, upwind)
     lam = np.polyfit(grow[:, 0], np.log(grow[:, 2]), 1)[0]
     print("dtype %s upwind %s" % ("f64" if dtype == binding.AC_F64 else "f32", upwind), end=" ")
     print("sigma %.0f: f0 %.4f Re_M %.3f (paper %.2f) lambda %.4e (paper %.2e)" % (sigma, f0, rem, rem_paper, lam, lam_paper))
-    assert abs(rem - rem_paper) <= 0.05 * rem_paper
+    # CALIBRATION check, not a comparison: f0 was tuned on the precursor runs until u_rms gives the printed Re_M
+    # (reading G23: Eq. 5 as printed, with f0 = 0.08, gives Re_M = 8.8, not the tables' 3.6), so this only says that
+    # the tuning converged.  The amplitude of Eq. 5 on the GPU path is pinned by parity with the oracle, whose own pin
+    # is P12 (box mean of |f|^2 = N^2 / 2).  The comparison with the paper is the growth rate below.
+    assert abs(rem - rem_paper) <= 0.05 * rem_paper, "f0 calibration did not converge"
     # the paper's own rows for this eta differ by 7 % between resolutions; one forcing realisation adds scatter
     assert abs(lam - lam_paper) <= 0.25 * abs(lam_paper)
     assert (lam > 0) == (sigma == 1.0)
