@@ -24,7 +24,7 @@ class OrcParams(ctypes.Structure):
         ("mixed_mode", ctypes.c_int), ("has_forcing", ctypes.c_int),
         ("fk", ctypes.c_double * 3), ("fphase", ctypes.c_double),
         ("fre", ctypes.c_double * 3), ("fim", ctypes.c_double * 3),
-        ("upwind", ctypes.c_int),
+        ("upwind", ctypes.c_int), ("forcing_kick", ctypes.c_int),
     ]
 
 
@@ -68,7 +68,7 @@ def _ptr(a):
 
 
 def make_params(shape, lengths, nu=0.0, eta=0.0, cs=1.0, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal",
-                upwind=False):
+                upwind=False, kick=False):
     nz, ny, nx = shape
     p = OrcParams()
     p.nx, p.ny, p.nz = nx, ny, nz
@@ -77,6 +77,7 @@ def make_params(shape, lengths, nu=0.0, eta=0.0, cs=1.0, forcing=None, bext=(0.0
     p.bext[:] = bext
     p.mixed_mode = {"bidiagonal": 0, "tensor": 1}[mixed]
     p.upwind = 1 if upwind else 0
+    p.forcing_kick = 1 if kick else 0
     if forcing is None:
         p.has_forcing = 0
     else:
@@ -97,10 +98,12 @@ def rhs(state, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="
     return out
 
 
-def step(state, dt, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal", upwind=False):
-    """One full RK3 step; returns a new array."""
+def step(state, dt, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal", upwind=False,
+         kick=False):
+    """One full RK3 step; returns a new array.  kick=True: the alternative reading of G8 (forcing as one impulse
+    u += dt f after the last substep instead of a term of the RHS in all three)."""
     state = np.array(state, dtype=np.float64, order="C", copy=True)
-    p = make_params(state.shape[1:], lengths, nu, eta, cs, forcing, bext, mixed, upwind)
+    p = make_params(state.shape[1:], lengths, nu, eta, cs, forcing, bext, mixed, upwind, kick)
     w = np.empty_like(state)
     scratch = np.empty_like(state)
     lib().orc_step(_ptr(state), _ptr(w), _ptr(scratch), float(dt), ctypes.byref(p))

@@ -206,11 +206,18 @@ def substep(state, w, s, dt, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0,
     return state + RK_BETA[s] * w, w
 
 
-def step(state, dt, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal", upwind=False):
-    """One full RK3 step (three substeps, same forcing parameters in all three: reading G8)."""
+def step(state, dt, lengths, nu, eta, cs, forcing=None, bext=(0.0, 0.0, 0.0), mixed="bidiagonal", upwind=False,
+         kick=False):
+    """One full RK3 step (three substeps, same forcing parameters in all three: reading G8).  kick=True is the
+    alternative reading: no forcing inside the substeps, one impulse u += dt f after the last one."""
     w = np.zeros_like(state)
     for s in range(3):
-        state, w = substep(state, w, s, dt, lengths, nu, eta, cs, forcing, bext, mixed, upwind)
+        state, w = substep(state, w, s, dt, lengths, nu, eta, cs, None if kick else forcing, bext, mixed, upwind)
+    if kick and forcing is not None:
+        state = state.copy()
+        f = forcing_field(state.shape[1:], grid_spacing(state.shape[1:], lengths), forcing)
+        for i in range(3):
+            state[UX + i] = state[UX + i] + dt * f[i]
     return state
 
 

@@ -57,6 +57,8 @@ typedef struct {
     int has_forcing;
     double fk[3], fphase, fre[3], fim[3];
     int upwind;          /* 0 = off (default, all BASELINE configs), 1 = upwinded continuity equation (G17) */
+    int forcing_kick;    /* 0 = f is a term of the RHS in all three substeps (default, reading G8); 1 = the alternative
+                            reading: the delta-correlated forcing is an impulse u += dt f added once, after substep 2 */
 } orc_params;
 
 static const double C1[3] = {3.0 / 4.0, -3.0 / 20.0, 1.0 / 60.0};
@@ -197,7 +199,7 @@ void orc_rhs(const double* state, double* rhs, const orc_params* p) {
                     for (int a = 0; a < 3; a++) rhs[c] += fabs(uc[a]) * der6_upwind(lnrho, p, x, y, z, a);
                 /* forcing, Eq. 4 */
                 double f[3] = {0.0, 0.0, 0.0};
-                if (p->has_forcing) {
+                if (p->has_forcing && !p->forcing_kick) {
                     double theta = p->fk[0] * (x * hx) + p->fk[1] * (y * hy) + p->fk[2] * (z * hz) + p->fphase;
                     double ct = cos(theta), st = sin(theta);
                     for (int i = 0; i < 3; i++) f[i] = p->fre[i] * ct - p->fim[i] * st;
@@ -236,6 +238,19 @@ void orc_step(double* state, double* w, double* scratch, double dt, const orc_pa
     const size_t n7 = (size_t)7 * p->nx * p->ny * p->nz;
     for (size_t i = 0; i < n7; i++) w[i] = 0.0;
     for (int s = 0; s < 3; s++) orc_substep(state, w, scratch, s, dt, p);
+    if (p->has_forcing && p->forcing_kick) {
+        /* alternative reading of G8: u += dt f(x) once per step, Eq. 4 evaluated as in orc_rhs */
+        const size_t n = (size_t)p->nx * p->ny * p->nz;
+        const double hx = spacing(p, 0), hy = spacing(p, 1), hz = spacing(p, 2);
+        for (long z = 0; z < p->nz; z++)
+            for (long y = 0; y < p->ny; y++)
+                for (long x = 0; x < p->nx; x++) {
+                    const size_t c = (size_t)x + (size_t)p->nx * ((size_t)y + (size_t)p->ny * (size_t)z);
+                    double theta = p->fk[0] * (x * hx) + p->fk[1] * (y * hy) + p->fk[2] * (z * hz) + p->fphase;
+                    double ct = cos(theta), st = sin(theta);
+                    for (int i = 0; i < 3; i++) state[(size_t)(1 + i) * n + c] += dt * (p->fre[i] * ct - p->fim[i] * st);
+                }
+    }
 }
 
 /* out: urms, umax, brms, bmax, lnrho_min, lnrho_max, nonfinite (0/1) */

@@ -105,7 +105,7 @@ template <typename E>
 __device__ __forceinline__ void q_st1(uint32_t taddr, E a) {
     uint32_t r[2];
     q_split(a, r[0], r[1]);
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(r[0]), "r"(r[1]) : "memory");
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(r[0]), "r"(r[1]));
 }
 // wider stores as single-element stores: a tcgen05.st.x8 wants its 8 source registers consecutive, which cost 8 moves
 // per store in the loop; x2 stores take each 8-byte value where it was computed
@@ -126,17 +126,15 @@ __device__ __forceinline__ void q_st4(uint32_t taddr, E a, E b, E c, E d) {
 __device__ __forceinline__ void q_ld8(uint32_t taddr, uint32_t (&r)[8]) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-                 : "r"(taddr)
-                 : "memory");
+                 : "r"(taddr));
 }
 __device__ __forceinline__ void q_ld4(uint32_t taddr, uint32_t (&r)[4]) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
-                 : "r"(taddr)
-                 : "memory");
+                 : "r"(taddr));
 }
 __device__ __forceinline__ void q_ld2(uint32_t taddr, uint32_t (&r)[2]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(taddr) : "memory");
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(taddr));
 }
 __device__ __forceinline__ void q_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void q_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
@@ -145,7 +143,7 @@ __device__ __forceinline__ void q_fence_after() { asm volatile("tcgen05.fence::a
 template <int N>
 __device__ __forceinline__ void q_tie(uint32_t (&r)[N]) {
 #pragma unroll
-    for (int i = 0; i < N; i++) asm volatile("" : "+r"(r[i])::"memory");
+    for (int i = 0; i < N; i++) asm volatile("" : "+r"(r[i]));
 }
 
 // ---- the in-plane neighbourhood of a column pair ----------------------------------------------------

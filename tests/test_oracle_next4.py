@@ -7,6 +7,9 @@ P20  the 2N-RK3 coefficients (G7) satisfy ALL four third-order conditions (Butch
      exact rationals: b = (1/6, 3/10, 8/15), c = (0, 1/3, 3/4)), and the full NON-LINEAR step converges with order 3
      (error ratio ~8 under dt halving against a dt/16 run): the condition sum b_i c_i^2 = 1/3 never enters a
      linear test.
+P22  the alternative reading of G8 (forcing as one impulse per step, oracle flag kick=True): from a zero state the
+     step returns exactly u = dt f(x) (Eq. 4 evaluated directly, nothing else touched); on a moving state the two
+     readings differ, at O(dt^2) (the coupling of f with the other terms inside the substeps); C against numpy.
 P21  the tensor-product reading of the mixed derivative (oracle flag mixed="tensor", G2) has the symbol
      -k1~(a) k1~(b) on a Fourier mode.
 """
@@ -137,3 +140,34 @@ def test_p21_tensor_product_mixed_derivative_symbol(impl, a, b):
     if impl == "numpy":
         bid = mn.dermix(f, a, b, h)
         assert np.abs(bid - want).max() > 1e-6
+
+
+@pytest.mark.parametrize("impl", ["c", "numpy"])
+def test_p22_forcing_as_one_impulse_per_step(impl):
+    from oracle import forcing as of
+    shape = (8, 10, 12)
+    lengths = (2 * math.pi, 1.5 * math.pi, 2.5 * math.pi)
+    dt = 2e-3
+    f = of.forcing_from_draws(0.37, 0.81, 0.12, 3, 1.0, dt, 0.05, 1.0, lengths)
+    step = mhd_c.step if impl == "c" else mn.step
+    zero = np.zeros((7,) + shape)
+    got = step(zero, dt, lengths, 1e-2, 1e-2, 1.0, f, kick=True)
+    # Eq. 4 written out here: f_i = re_i cos(k.x + phase) - im_i sin(k.x + phase)
+    k, phase, re, im = f
+    nz, ny, nx = shape
+    x = np.arange(nx) * (lengths[0] / nx)
+    y = np.arange(ny) * (lengths[1] / ny)
+    z = np.arange(nz) * (lengths[2] / nz)
+    th = k[0] * x[None, None, :] + k[1] * y[None, :, None] + k[2] * z[:, None, None] + phase
+    amp = max(np.abs(re).max(), np.abs(im).max())
+    for i in range(3):
+        assert np.abs(got[1 + i] - dt * (re[i] * np.cos(th) - im[i] * np.sin(th))).max() <= 1e-15 * dt * amp
+    assert np.abs(got[0]).max() == 0.0 and np.abs(got[4:]).max() == 0.0
+    # on a moving state the readings differ, but only at second order in dt
+    state = inputs.smooth_strong_state(shape, 9)
+    a = step(state, dt, lengths, 1e-2, 1e-2, 1.0, f)
+    b = step(state, dt, lengths, 1e-2, 1e-2, 1.0, f, kick=True)
+    gap = np.abs(a[1:4] - b[1:4]).max()
+    assert 0.0 < gap < 20 * dt * dt * amp
+    if impl == "c":
+        assert np.abs(b - mn.step(state, dt, lengths, 1e-2, 1e-2, 1.0, f, kick=True)).max() < 1e-15
