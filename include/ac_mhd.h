@@ -221,6 +221,12 @@ int ac_set_bext(ac_ctx* ctx, const double b[3]);
  * + sum_a |u_a| / (60 h_a) [f(-3) - 6 f(-2) + 15 f(-1) - 20 f(0) + 15 f(+1) - 6 f(+2) + f(+3)],
  * which makes each u_a d_a ln rho the 5th-order upwind-biased derivative.  Default 0. */
 int ac_set_upwind(ac_ctx* ctx, int on);
+/* ac_set_forcing_mode: how the forcing of Eq. 4 enters the three substeps, which the paper does not say (G8).
+ * 0 (default, every reported number) = f is a term of the right-hand side in all three substeps; 1 = the forcing is
+ * delta-correlated and acts as ONE impulse u += dt f per time step, after the last substep (the
+ * Pencil-Code convention behind Eq. 5's dt^-1/2).  The net impulse is the same, the O(dt^2) coupling terms differ.
+ * Not between the substeps of a step (AC_ESTATE). */
+int ac_set_forcing_mode(ac_ctx* ctx, int mode);
 /* ac_set_mixed: reading of the mixed-derivative scheme, which the paper does not print (G2).  0 (default, all
  * reported parity and every BASELINE config) = bidiagonal 12-point stencil; 1 = tensor product D_a(D_b f), 36
  * points, also radius 3 and 6th order.  Mode 1 runs the direct kernel whatever the variant.  Like ac_set_variant

@@ -21,7 +21,7 @@ EXPORTS = (
     "ac_forcing_from_draws", "ac_forcing_params", "ac_make_forcing", "ac_set_bext", "ac_set_cfl", "ac_set_variant",
     "ac_set_upwind", "ac_set_mixed", "ac_substep", "ac_state_layout", "ac_field_device_ptr", "ac_reduce_raw",
     "ac_reduce_ext", "ac_reduce_ext_raw", "ac_set_slab", "ac_substep_part", "ac_halo_bytes", "ac_halo_pack",
-    "ac_halo_unpack", "ac_diag_combine",
+    "ac_halo_unpack", "ac_diag_combine", "ac_set_forcing_mode",
     "ac_launch_count", "ac_free", "ac_strerror", "ac_version",
 )
 
@@ -121,6 +121,8 @@ def load_library():
     L.ac_reduce_ext.restype = i32
     L.ac_reduce_ext_raw.argtypes = [vp, ctypes.POINTER(dbl)]
     L.ac_reduce_ext_raw.restype = i32
+    L.ac_set_forcing_mode.argtypes = [vp, i32]
+    L.ac_set_forcing_mode.restype = i32
     L.ac_set_slab.argtypes = [vp, i32, i32]
     L.ac_set_slab.restype = i32
     L.ac_substep_part.argtypes = [vp, i32, dbl, ctypes.POINTER(AcForcing), i32]
@@ -366,6 +368,11 @@ class Context:
 
     def ac_set_upwind(self, on):
         _check(self._lib.ac_set_upwind(self._ctx, int(bool(on))), "ac_set_upwind")
+
+    def ac_set_forcing_mode(self, mode):
+        """0 / "rhs" (default, reading G8) or 1 / "kick" (one impulse u += dt f per step)."""
+        mode = {"rhs": 0, "kick": 1}.get(mode, mode)
+        _check(self._lib.ac_set_forcing_mode(self._ctx, int(mode)), "ac_set_forcing_mode")
 
     def ac_set_mixed(self, mode):
         """0 / "bidiagonal" (default) or 1 / "tensor"."""

@@ -144,6 +144,7 @@ struct ac_ctx {
     double bext[3];
     double c_u, c_nu;
     int upwind;          // 1 = upwinded continuity equation (G17); default 0
+    int forcing_kick;    // 1 = alternative reading of G8: one impulse u += dt f per step, applied with substep 2; default 0
     int mixed;           // 0 = bidiagonal mixed stencil (G2, default), 1 = tensor product (direct kernel only)
     int variant;         // requested: 0 = pair-march (default), 1 = direct, 2 = scatter-march (one cell per thread)
     bool march;          // the kernel actually used (fp32 with odd nz falls back to direct)
@@ -334,6 +335,23 @@ int substep_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s, int part
     const ac::Layout& L = ctx->L;
     const ac_grid& g = ctx->grid;
     T* ftab = (T*)(ctx->ws + ctx->cv.ftab_off);
+    ac_forcing kick;
+    if (forcing && ctx->forcing_kick) {
+        // alternative reading of G8: nothing in substeps 0 and 1; substep 2 is the last update of the step, and its
+        // 2N register is never used again (alpha_0 = 0), so adding f / beta_2 to its right-hand side IS the impulse
+        // u += dt f after the step
+        if (s < 2) {
+            forcing = nullptr;
+        } else {
+            kick = *forcing;
+            for (int i = 0; i < 3; i++) {
+                kick.re[i] /= RK_BETA[2];
+                kick.im[i] /= RK_BETA[2];
+            }
+            forcing = &kick;
+            tables = true;
+        }
+    }
     if (forcing && part != PART_OUTER && tables) {
         // a slab sees the global wave with its own origin: phase + k_z z0 (Eq. 4)
         const double hz = g.lz / g.nz;
@@ -701,6 +719,7 @@ int ac_init(ac_ctx** out, const ac_grid* grid, ac_dtype dtype, double nu, double
     ctx->c_nu = 0.25;
     ctx->variant = 0;
     ctx->upwind = 0;
+    ctx->forcing_kick = 0;
     ctx->mixed = 0;
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->launches = 0;
@@ -1090,6 +1109,13 @@ int ac_set_cfl(ac_ctx* ctx, double c_u, double c_nu) {
 int ac_set_upwind(ac_ctx* ctx, int on) {
     if (!ctx || (on != 0 && on != 1)) return AC_EINVAL;
     ctx->upwind = on;
+    return AC_OK;
+}
+
+int ac_set_forcing_mode(ac_ctx* ctx, int mode) {
+    if (!ctx || (mode != 0 && mode != 1)) return AC_EINVAL;
+    if (ctx->next_substep != 0 || ctx->inner_done != -1) return AC_ESTATE;
+    ctx->forcing_kick = mode;
     return AC_OK;
 }
 

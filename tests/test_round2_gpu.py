@@ -110,3 +110,33 @@ def test_config3_256cubed_full_field_one_step(dtype):
     err = helpers.group_errors(got, want)
     print("256^3 full field", npdt.__name__, err)
     assert max(err.values()) <= (1e-12 if dtype == binding.AC_F64 else 1e-5)
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("dtype", [binding.AC_F64, binding.AC_F32])
+def test_forcing_as_one_impulse_per_step(variant, dtype):
+    """the alternative reading of G8 (ac_set_forcing_mode("kick")) against the oracle's kick=True,
+    two steps on a moving state; and it is not the default reading."""
+    shape = (24, 40, 32)
+    lengths = (2 * math.pi, 1.6 * math.pi, 2.2 * math.pi)
+    npdt = np.float64 if dtype == binding.AC_F64 else np.float32
+    state = inputs.smooth_strong_state(shape, 33).astype(npdt)
+    nu, eta, dt = 2e-2, 1e-2, 2e-3
+    ctx = binding.Context(shape, lengths, dtype, nu=nu, eta=eta, k_f=3, helicity=1.0)
+    ctx.ac_set_variant(variant)
+    ctx.ac_set_forcing_mode("kick")
+    ctx.ac_load_state(state)
+    want = state.astype(np.float64)
+    other = want
+    for s in range(2):
+        f = helpers.oracle_forcing(9, s, 3, 1.0, dt, 0.05, 1.0, lengths)
+        ctx.ac_step(dt, ctx.ac_make_forcing(9, s, dt, 0.05))
+        want = mhd_c.step(want, dt, lengths, nu, eta, 1.0, f, kick=True)
+        other = mhd_c.step(other, dt, lengths, nu, eta, 1.0, f)
+    got = ctx.ac_store_state()
+    ctx.ac_free()
+    err = helpers.max_group_error(got, want)
+    gap = helpers.max_group_error(other, want)
+    print("kick reading", variant, npdt.__name__, err, "kick vs rhs", gap)
+    assert err <= (2e-12 if dtype == binding.AC_F64 else 1e-5)
+    assert gap > 100 * err or dtype == binding.AC_F32
