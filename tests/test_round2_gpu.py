@@ -140,3 +140,25 @@ def test_forcing_as_one_impulse_per_step(variant, dtype):
     print("kick reading", variant, npdt.__name__, err, "kick vs rhs", gap)
     assert err <= (2e-12 if dtype == binding.AC_F64 else 1e-5)
     assert gap > 100 * err or dtype == binding.AC_F32
+
+
+def test_config3_256cubed_ten_steps_fp64():
+    """north_star: fp64 within 1e-9 of the oracle after 10 steps on the same seeded inputs, on EVERY cell of the
+    256^3 box of BASELINE config 3 (about two minutes of oracle on 16 cores); forcing redrawn every step."""
+    n = 256
+    nu, seed = 1e-3, 1003
+    state = inputs.solenoidal_state(n, seed)
+    ctx = binding.Context((n, n, n), TWO_PI3, binding.AC_F64, nu=nu, eta=nu, cs=1.0, k_f=3, helicity=0.0)
+    ctx.ac_load_state(state)
+    h = 2 * math.pi / n
+    umax = float(np.sqrt((state[1:4] ** 2).sum(axis=0).max()))
+    dt = 0.8 * min(0.4 * h / (umax + 1.0), 0.25 * h * h / nu)       # fixed, from the oracle side
+    st = mhd_c.Stepper(state, TWO_PI3, nu, nu, 1.0)
+    for s in range(10):
+        ctx.ac_step(dt, ctx.ac_make_forcing(seed + 7, s, dt, 0.02))
+        st.step(dt, helpers.oracle_forcing(seed + 7, s, 3, 0.0, dt, 0.02, 1.0))
+    got = ctx.ac_store_state()
+    ctx.ac_free()
+    err = helpers.group_errors(got, st.state)
+    print("256^3, 10 steps, fp64:", err)
+    assert max(err.values()) <= 1e-9
