@@ -50,6 +50,52 @@ struct RqLanes<f2> {
     }
 };
 
+// running extrema in the element's own precision: exact, and one FMNMX per lane instead of an fp64 compare-select
+template <typename E>
+struct RqExt;
+template <>
+struct RqExt<double> {
+    double mu = 0.0, mb = 0.0, lmin = INFINITY, lmax = -INFINITY;
+    __device__ void umax(double v) { mu = fmax(mu, v); }
+    __device__ void bmax(double v) { mb = fmax(mb, v); }
+    __device__ void lminmax(double v) {
+        lmin = fmin(lmin, v);
+        lmax = fmax(lmax, v);
+    }
+    __device__ void fold(RedVals& a) const {
+        a.mu = fmax(a.mu, mu);
+        a.mb = fmax(a.mb, mb);
+        a.lmin = fmin(a.lmin, lmin);
+        a.lmax = fmax(a.lmax, lmax);
+    }
+};
+template <>
+struct RqExt<f2> {
+    float mu = 0.f, mb = 0.f, lmin = INFINITY, lmax = -INFINITY;
+    __device__ void umax(f2 v) {
+        float lo, hi;
+        vunpack(v, lo, hi);
+        mu = fmaxf(mu, fmaxf(lo, hi));
+    }
+    __device__ void bmax(f2 v) {
+        float lo, hi;
+        vunpack(v, lo, hi);
+        mb = fmaxf(mb, fmaxf(lo, hi));
+    }
+    __device__ void lminmax(f2 v) {
+        float lo, hi;
+        vunpack(v, lo, hi);
+        lmin = fminf(lmin, fminf(lo, hi));
+        lmax = fmaxf(lmax, fmaxf(lo, hi));
+    }
+    __device__ void fold(RedVals& a) const {
+        a.mu = fmax(a.mu, (double)mu);
+        a.mb = fmax(a.mb, (double)mb);
+        a.lmin = fmin(a.lmin, (double)lmin);
+        a.lmax = fmax(a.lmax, (double)lmax);
+    }
+};
+
 template <typename T, int LANES>
 __global__ void __launch_bounds__(RQ_THREADS, 3)
     reduce_tma_kernel(const __grid_constant__ ReduceArgs<T> a, const __grid_constant__ CUtensorMap map_a,
@@ -97,6 +143,7 @@ __global__ void __launch_bounds__(RQ_THREADS, 3)
 
     // -------------------------------------------- workers --------------------------------------------
     RedVals acc = red_identity();
+    RqExt<E> ext;
     const int tx = tid & (M_TX - 1), ty = tid >> 4;
     const int cell_off = ((ty + R) * M_WX + tx + M_HX) * 8;           // bytes
     E c1[3][3], bext[3];
@@ -119,76 +166,80 @@ __global__ void __launch_bounds__(RQ_THREADS, 3)
         for (int r = 0; r < 7; r++) hax[r] = hay[r] = vzero<E>();
 #pragma unroll
         for (int r = 0; r < 4; r++) pbx[r] = pby[r] = pbz[r] = vzero<E>();
+        // the plane loop is unrolled 7 x so that the 7-plane history of A_x, A_y is a rotating register file with
+        // compile-time indices (no moves): plane k sits in slot k % 7, H(r) = plane k - 6 + r
 #pragma unroll 1
-        for (int k = 0; k < niter; k++, it++) {
-            const int slot = (int)(it % RQ_NP);
+        for (int k0 = 0; k0 < niter; k0 += 7) {
 #pragma unroll
-            for (int r = 0; r < 6; r++) {
-                hax[r] = hax[r + 1];
-                hay[r] = hay[r + 1];
-            }
+            for (int j = 0; j < 7; j++) {
+                const int k = k0 + j;
+                if (k >= niter) break;
+#define RQ_H(arr, r) arr[(j + 1 + (r)) % 7]
+                const int slot = (int)(it % RQ_NP);
 #pragma unroll
-            for (int r = 0; r < 3; r++) {
-                pbx[r] = pbx[r + 1];
-                pby[r] = pby[r + 1];
-                pbz[r] = pbz[r + 1];
-            }
-            m_bar_wait<0>(&full[slot], (uint32_t)((it / RQ_NP) & 1));
-            const unsigned char* p0 = rq_smem + slot * RQ_SLOT_BYTES + cell_off;
-            hax[6] = rq_lds<E>(p0);
-            hay[6] = rq_lds<E>(p0 + M_PLANE * 8);
-            if (k >= R && k < niter - R && valid) {
-                // the plane is one of the item's own: in-plane parts of B, and the pointwise fields
-                auto din = [&](int f, int stride, int axis) -> E {
-                    const unsigned char* p = p0 + f * (M_PLANE * 8);
-                    E r = vmul(c1[axis][0], vsub(rq_lds<E>(p + stride), rq_lds<E>(p - stride)));
-                    r = vfma(c1[axis][1], vsub(rq_lds<E>(p + 2 * stride), rq_lds<E>(p - 2 * stride)), r);
-                    r = vfma(c1[axis][2], vsub(rq_lds<E>(p + 3 * stride), rq_lds<E>(p - 3 * stride)), r);
-                    return r;
-                };
-                pbx[3] = din(2, M_WX * 8, 1);
-                pby[3] = din(2, 8, 0);
-                pbz[3] = vadd(vsub(din(1, 8, 0), din(0, M_WX * 8, 1)), bext[2]);
-                const E az = rq_lds<E>(p0 + 2 * M_PLANE * 8);
-                const unsigned char* pp = rq_smem + RQ_OFF_P + slot * RQ_PSLOT_BYTES + tid * 8;
-                // |u|^2 in the element's own arithmetic (fp64, or packed fp32: the squares are rounded to fp32, reading
-                // G18), sums and extrema in fp64
-                const E vx = rq_lds<E>(pp + M_COLS * 8), vy = rq_lds<E>(pp + 2 * M_COLS * 8), vz = rq_lds<E>(pp + 3 * M_COLS * 8);
-                const E lr = rq_lds<E>(pp);
-                double l[2], u2[2], chk[2];
-                RqLanes<E>::get(lr, l);
-                RqLanes<E>::get(vfma(vz, vz, vfma(vy, vy, vmul(vx, vx))), u2);
-                // a non-finite ln rho or A would hide in fmin/fmax: fold it into the sums
-                RqLanes<E>::get(vadd(vadd(vadd(hax[6], hay[6]), az), lr), chk);
-#pragma unroll
-                for (int i = 0; i < LANES; i++) {
-                    acc.su += u2[i];
-                    acc.mu = fmax(acc.mu, u2[i]);
-                    acc.lmin = fmin(acc.lmin, l[i]);
-                    acc.lmax = fmax(acc.lmax, l[i]);
-                    if (!isfinite(chk[i])) acc.su += chk[i];
+                for (int r = 0; r < 3; r++) {
+                    pbx[r] = pbx[r + 1];
+                    pby[r] = pby[r + 1];
+                    pbz[r] = pbz[r + 1];
                 }
-            }
-            if (k >= 2 * R && valid) {                                // plane p - 3 has its 7-plane history: finish B there
-                E ayz = vmul(c1[2][0], vsub(hay[4], hay[2]));
-                ayz = vfma(c1[2][1], vsub(hay[5], hay[1]), ayz);
-                ayz = vfma(c1[2][2], vsub(hay[6], hay[0]), ayz);
-                E axz = vmul(c1[2][0], vsub(hax[4], hax[2]));
-                axz = vfma(c1[2][1], vsub(hax[5], hax[1]), axz);
-                axz = vfma(c1[2][2], vsub(hax[6], hax[0]), axz);
-                const E bx = vadd(vsub(pbx[0], ayz), bext[0]), by = vadd(vsub(axz, pby[0]), bext[1]), bz = pbz[0];
-                double b2[2];
-                RqLanes<E>::get(vfma(bz, bz, vfma(by, by, vmul(bx, bx))), b2);
+                m_bar_wait<0>(&full[slot], (uint32_t)((it / RQ_NP) & 1));
+                const unsigned char* p0 = rq_smem + slot * RQ_SLOT_BYTES + cell_off;
+                RQ_H(hax, 6) = rq_lds<E>(p0);
+                RQ_H(hay, 6) = rq_lds<E>(p0 + M_PLANE * 8);
+                if (k >= R && k < niter - R && valid) {
+                    // the plane is one of the item's own: in-plane parts of B, and the pointwise fields
+                    auto din = [&](int f, int stride, int axis) -> E {
+                        const unsigned char* p = p0 + f * (M_PLANE * 8);
+                        E r = vmul(c1[axis][0], vsub(rq_lds<E>(p + stride), rq_lds<E>(p - stride)));
+                        r = vfma(c1[axis][1], vsub(rq_lds<E>(p + 2 * stride), rq_lds<E>(p - 2 * stride)), r);
+                        r = vfma(c1[axis][2], vsub(rq_lds<E>(p + 3 * stride), rq_lds<E>(p - 3 * stride)), r);
+                        return r;
+                    };
+                    pbx[3] = din(2, M_WX * 8, 1);
+                    pby[3] = din(2, 8, 0);
+                    pbz[3] = vadd(vsub(din(1, 8, 0), din(0, M_WX * 8, 1)), bext[2]);
+                    const E az = rq_lds<E>(p0 + 2 * M_PLANE * 8);
+                    const unsigned char* pp = rq_smem + RQ_OFF_P + slot * RQ_PSLOT_BYTES + tid * 8;
+                    // |u|^2 in the element's own arithmetic (fp64, or packed fp32: the squares are rounded to fp32,
+                    // reading G18); sums in fp64; extrema in the element's precision (exact) until the fold
+                    const E vx = rq_lds<E>(pp + M_COLS * 8), vy = rq_lds<E>(pp + 2 * M_COLS * 8), vz = rq_lds<E>(pp + 3 * M_COLS * 8);
+                    const E lr = rq_lds<E>(pp);
+                    const E u2 = vfma(vz, vz, vfma(vy, vy, vmul(vx, vx)));
+                    ext.umax(u2);
+                    ext.lminmax(lr);
+                    double u2d[2], chk[2];
+                    RqLanes<E>::get(u2, u2d);
+                    // a non-finite ln rho or A would hide in the extrema: fold it into the sums
+                    RqLanes<E>::get(vadd(vadd(vadd(RQ_H(hax, 6), RQ_H(hay, 6)), az), lr), chk);
 #pragma unroll
-                for (int i = 0; i < LANES; i++) {
-                    acc.sb += b2[i];
-                    acc.mb = fmax(acc.mb, b2[i]);
+                    for (int i = 0; i < LANES; i++) {
+                        acc.su += u2d[i];
+                        if (!isfinite(chk[i])) acc.su += chk[i];
+                    }
                 }
+                if (k >= 2 * R && valid) {                            // plane p - 3 has its 7-plane history: finish B there
+                    E ayz = vmul(c1[2][0], vsub(RQ_H(hay, 4), RQ_H(hay, 2)));
+                    ayz = vfma(c1[2][1], vsub(RQ_H(hay, 5), RQ_H(hay, 1)), ayz);
+                    ayz = vfma(c1[2][2], vsub(RQ_H(hay, 6), RQ_H(hay, 0)), ayz);
+                    E axz = vmul(c1[2][0], vsub(RQ_H(hax, 4), RQ_H(hax, 2)));
+                    axz = vfma(c1[2][1], vsub(RQ_H(hax, 5), RQ_H(hax, 1)), axz);
+                    axz = vfma(c1[2][2], vsub(RQ_H(hax, 6), RQ_H(hax, 0)), axz);
+                    const E bx = vadd(vsub(pbx[0], ayz), bext[0]), by = vadd(vsub(axz, pby[0]), bext[1]), bz = pbz[0];
+                    const E b2 = vfma(bz, bz, vfma(by, by, vmul(bx, bx)));
+                    ext.bmax(b2);
+                    double b2d[2];
+                    RqLanes<E>::get(b2, b2d);
+#pragma unroll
+                    for (int i = 0; i < LANES; i++) acc.sb += b2d[i];
+                }
+                __syncwarp();
+                if (lane == 0) m_bar_arrive(&done[slot]);
+                it++;
+#undef RQ_H
             }
-            __syncwarp();
-            if (lane == 0) m_bar_arrive(&done[slot]);
         }
     }
+    ext.fold(acc);
     // fold the 4 worker warps (the producer warp has left: no __syncthreads here)
     __shared__ RedVals warp_part[RQ_WORKERS / 32];
 #pragma unroll
