@@ -362,7 +362,9 @@ def run_slab(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     else:
-        dist.init_process_group("gloo", init_method="tcp://127.0.0.1:29561", rank=0, world_size=1)
+        # one rank: NCCL still carries the halo (the rank sends to itself), so the transport path is the real one
+        dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29561", rank=0, world_size=1,
+                                device_id=torch.device("cuda", local_rank))
     rank = dist.get_rank()
     n = args.n
     cfg = workload(n)

@@ -208,10 +208,12 @@ class SlabRank:
         return self.slab.ctx.ac_forcing_from_draws(u1, u2, u3, dt, f0)
 
     def transfer(self):
-        if self.world > 1:
+        if self.world > 1 or self.dist.get_backend() == "nccl":
+            # with one rank NCCL sends to itself (the rank is its own neighbour above and below): the same
+            # stream-ordered code path as between GPUs
             transfer_distributed(self.slab, self.dist)
         else:
-            transfer_in_process([self.slab])                  # a single rank is its own neighbour
+            transfer_in_process([self.slab])
 
     def exchange(self):
         self.slab.pack()

@@ -1,5 +1,7 @@
-"""Worker of tests/test_slab_gpu.py::test_slab_ranks_as_processes: one rank of a z-slab run (torchrun, gloo; the
-ranks share cuda:0, which is safe because no kernel waits on another rank: the exchange is host-synchronised)."""
+"""Worker of tests/test_slab_gpu.py: one rank of a z-slab run under torchrun.  gloo: two ranks share cuda:0 (safe: no
+kernel waits on another rank, the exchange is staged through the host).  nccl: ONE rank, which is its own neighbour
+above and below, so that the stream-ordered NCCL transport (slab.ring_transfer on the communication stream, no host
+synchronisation) runs for real on one GPU."""
 import math
 import os
 import sys
@@ -14,7 +16,13 @@ from paper_2012_08758_b200 import binding, inputs, slab  # noqa: E402
 
 def main():
     out_dir = sys.argv[1]
-    dist.init_process_group("gloo")
+    backend = sys.argv[2] if len(sys.argv) > 2 else "gloo"
+    if backend == "nccl":
+        import torch
+        torch.cuda.set_device(0)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", 0))
+    else:
+        dist.init_process_group("gloo")
     shape = (32, 24, 32)
     lengths = (2 * math.pi, 1.5 * math.pi, 3.0 * math.pi)
     state = inputs.smooth_strong_state(shape, 41)

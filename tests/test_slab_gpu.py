@@ -112,3 +112,32 @@ def test_slab_ranks_as_processes(tmp_path):
     assert err <= 1e-13
     for v, key in zip(diag, ("urms", "brms", "umax", "bmax", "dt_cfl")):
         assert abs(v - d[key]) <= 1e-12 * abs(d[key]), key
+
+
+def test_slab_rank_over_nccl_with_one_rank(tmp_path):
+    """The NCCL transport on one GPU: a single rank is its own neighbour above and below, so slab.SlabRank sends its
+    halo buffers to itself through ncclSend / ncclRecv on the communication stream, overlapped with the inner part,
+    exactly as between GPUs.  Must equal the ordinary periodic context."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "1", "--master-addr",
+           "127.0.0.1", "--master-port", "29553", os.path.join(root, "tests", "slab_worker.py"), str(tmp_path), "nccl"]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=root)
+    assert r.returncode == 0, r.stderr[-3000:]
+    got = np.load(tmp_path / "slab_0.npy")
+    shape = (32, 24, 32)
+    lengths = (2 * math.pi, 1.5 * math.pi, 3.0 * math.pi)
+    one = binding.Context(shape, lengths, binding.AC_F64, nu=5e-3, eta=4e-3, cs=1.0, k_f=3, helicity=1.0)
+    one.ac_load_state(inputs.smooth_strong_state(shape, 41))
+    dt = 2e-3
+    for s in range(2):
+        one.ac_step(dt, one.ac_forcing_from_draws(0.3 + 0.1 * s, 0.6, 0.2, dt, 0.02))
+    want = one.ac_store_state()
+    d = one.ac_reduce()
+    diag = np.load(tmp_path / "diag.npy")
+    one.ac_free()
+    assert np.array_equal(got, want)
+    for v, key in zip(diag, ("urms", "brms", "umax", "bmax", "dt_cfl")):
+        assert abs(v - d[key]) <= 1e-13 * abs(d[key]), key
