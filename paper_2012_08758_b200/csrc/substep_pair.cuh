@@ -378,18 +378,6 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
         const bool valid_x = x < L.nx;
         if (warp < 4) {
             // =============================== U: ln rho, u ===============================
-            // forcing: cos/sin of k_x x + k_y y, constant along the march
-            E cxy[2], sxy[2];
-#pragma unroll
-            for (int cc = 0; cc < 2; cc++) {
-                cxy[cc] = sxy[cc] = vzero<E>();
-                if (a.has_forcing && valid_x && y + cc < L.ny) {
-                    const T cx_ = a.ftab[x], sx_ = a.ftab[L.nx + x];
-                    const T cy_ = a.ftab[2 * L.nx + y + cc], sy_ = a.ftab[2 * L.nx + L.ny + y + cc];
-                    cxy[cc] = Splat<E>::of((double)(cx_ * cy_ - sx_ * sy_));
-                    sxy[cc] = Splat<E>::of((double)(sx_ * cy_ + cx_ * sy_));
-                }
-            }
             E Lx[2][6], Ly[2][6], Lz[2][6], u6z[2][6];
             q_zero(Lx); q_zero(Ly); q_zero(Lz); q_zero(u6z);
             for (int k = 0; k < niter; k++) {
@@ -465,13 +453,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                     E Gxz[2], Gyz[2], uxc[2], uyc[2], gzc[2], Gzzc[2], lnc[2], uzc[2], unused0[2], unused1[2];
                     q_hist_gather<E, false, Q_UH_SLOT>(tm + Q_TM_UH + 8, k, c.c1z, c.c2z, c.c20z, Gxz, Gyz, unused0, unused1, uxc, uyc);
                     q_hist_gather<E, false, Q_UH_SLOT>(tm + Q_TM_UH, k, c.c1z, c.c2z, c.c20z, gzc, Gzzc, unused0, unused1, lnc, uzc);
-                    // forcing Eq. 4: f_i = re_i cos(theta) - im_i sin(theta)
-                    E cz_ = vzero<E>(), sz_ = vzero<E>();
-                    if (a.has_forcing) {
-                        cz_ = ztab[2 * (z - zs)];
-                        sz_ = ztab[2 * (z - zs) + 1];
-                    }
-                    // (j x B) / rho from the A role of the same columns
+                    // (j x B) / rho + f from the A role of the same columns
                     m_bar_wait<Q_WAIT_MAILBOX>(&mfull[wp * Q_ND + u % Q_ND], (uint32_t)((u / Q_ND) & 1));
                     q_fence_after();
 #pragma unroll
@@ -509,11 +491,6 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                             up = vfma(vabs(uy), u6y0, up);
                             rl = vadd(rl, vfma(vabs(uz), fu6z[cc], up));
                         }
-                        E fc = vzero<E>(), fs = vzero<E>();
-                        if (a.has_forcing) {
-                            fc = vsub(vmul(cxy[cc], cz_), vmul(sxy[cc], sz_));
-                            fs = vfma(sxy[cc], cz_, vmul(cxy[cc], sz_));
-                        }
                         // 2 S_ij g_j = (G_ij + G_ji) g_j - 2/3 div u g_i
                         const E sxy_ = vadd(Gxy0, Gyx0), sxz_ = vadd(Gxz0, Gzx0), syz_ = vadd(Gyz0, Gzy0);
                         const E dd = vmul(c.n23, divu);
@@ -542,11 +519,6 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                         E r0 = vfma(c.nu, vadd(fLx[cc], sg0), vadd(jxb0, vsub(vmul(c.ncs2, g0), adv0)));
                         E r1 = vfma(c.nu, vadd(fLy[cc], sg1), vadd(jxb1, vsub(vmul(c.ncs2, g1), adv1)));
                         E r2 = vfma(c.nu, vadd(fLz[cc], sg2), vadd(jxb2, vsub(vmul(c.ncs2, g2), adv2)));
-                        if (a.has_forcing) {
-                            r0 = vfma(c.fre[0], fc, vfma(c.nfim[0], fs, r0));
-                            r1 = vfma(c.fre[1], fc, vfma(c.nfim[1], fs, r1));
-                            r2 = vfma(c.fre[2], fc, vfma(c.nfim[2], fs, r2));
-                        }
                         // 2N-RK3 update, difference form
                         E o0 = lnrho, o1 = ux, o2 = uy, o3 = uz;
                         if (with_prev) {
@@ -575,6 +547,20 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
             }
         } else {
             // =============================== A: vector potential ===============================
+            // the forcing of Eq. 4 rides on the mailbox: the A role, which is not on the critical path, adds f_i to
+            // (j x B)_i / rho before it hands the sum over
+            // cos/sin of k_x x + k_y y, constant along the march
+            E cxy[2], sxy[2];
+#pragma unroll
+            for (int cc = 0; cc < 2; cc++) {
+                cxy[cc] = sxy[cc] = vzero<E>();
+                if (a.has_forcing && valid_x && y + cc < L.ny) {
+                    const T cx_ = a.ftab[x], sx_ = a.ftab[L.nx + x];
+                    const T cy_ = a.ftab[2 * L.nx + y + cc], sy_ = a.ftab[2 * L.nx + L.ny + y + cc];
+                    cxy[cc] = Splat<E>::of((double)(cx_ * cy_ - sx_ * sy_));
+                    sxy[cc] = Splat<E>::of((double)(sx_ * cy_ + cx_ * sy_));
+                }
+            }
             E Pz[2][6], Jx[2][6], Jy[2][6], Jz[2][6];
             q_zero(Pz); q_zero(Jx); q_zero(Jy); q_zero(Jz);
             const E c20xy = vneg(c.nc20xy);     // centre weight of D_xx + D_yy
@@ -636,6 +622,11 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                     // d_z and d_zz of A_x, A_y from the centre history
                     E dzax[2], dzay[2], zzax[2], zzay[2], axc[2], ayc[2];
                     q_hist_gather<E, true, Q_AH_SLOT>(tm + Q_TM_AH, k, c.c1z, c.c2z, c.c20z, dzax, dzay, zzax, zzay, axc, ayc);
+                    E cz_ = vzero<E>(), sz_ = vzero<E>();
+                    if (a.has_forcing) {
+                        cz_ = ztab[2 * (z - zs)];
+                        sz_ = ztab[2 * (z - zs) + 1];
+                    }
                     E b0[2], b1[2], b2[2], P0[2], P1[2];
 #pragma unroll
                     for (int cc = 0; cc < 2; cc++) {
@@ -656,10 +647,20 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                         P1[cc] = vadd(Pyip0, zzay[cc]);
                         const E j0 = vsub(fJx[cc], zzax[cc]), j1 = vsub(fJy[cc], zzay[cc]), j2 = fJz[cc];
                         const E rho_inv = vexpneg(pc[cc * Q_WX]);
+                        E m0 = vmul(rho_inv, vsub(vmul(j1, b2[cc]), vmul(j2, b1[cc])));
+                        E m1 = vmul(rho_inv, vsub(vmul(j2, b0[cc]), vmul(j0, b2[cc])));
+                        E m2 = vmul(rho_inv, vsub(vmul(j0, b1[cc]), vmul(j1, b0[cc])));
+                        if (a.has_forcing) {
+                            // forcing Eq. 4: f_i = re_i cos(theta) - im_i sin(theta)
+                            const E fc = vsub(vmul(cxy[cc], cz_), vmul(sxy[cc], sz_));
+                            const E fs = vfma(sxy[cc], cz_, vmul(cxy[cc], sz_));
+                            m0 = vfma(c.fre[0], fc, vfma(c.nfim[0], fs, m0));
+                            m1 = vfma(c.fre[1], fc, vfma(c.nfim[1], fs, m1));
+                            m2 = vfma(c.fre[2], fc, vfma(c.nfim[2], fs, m2));
+                        }
                         const uint32_t sm = tm + (uint32_t)(Q_TM_MB + ((u % Q_ND) * 2 + cc) * Q_MB_CELL);
-                        q_st2<E>(sm, vmul(rho_inv, vsub(vmul(j1, b2[cc]), vmul(j2, b1[cc]))),
-                                 vmul(rho_inv, vsub(vmul(j2, b0[cc]), vmul(j0, b2[cc]))));
-                        q_st1<E>(sm + 4, vmul(rho_inv, vsub(vmul(j0, b1[cc]), vmul(j1, b0[cc]))));
+                        q_st2<E>(sm, m0, m1);
+                        q_st1<E>(sm + 4, m2);
                     }
                     q_wait_st();
                     q_fence_before();
