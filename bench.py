@@ -378,7 +378,8 @@ def run_slab(args):
         npdt = np.float64 if dtype_name == "f64" else np.float32
         es = 8 if dtype_name == "f64" else 4
         rk = slab.SlabRank((nz_global, n, n), lengths, dist, dtype, device="cuda:%d" % local_rank, variant=args.variant,
-                           overlap=not args.no_overlap, nu=nu, eta=nu, cs=1.0, k_f=3.0, helicity=cfg["sigma"])
+                           overlap=not args.no_overlap, transport="pull" if args.transport == "pull" else "buffers",
+                           nu=nu, eta=nu, cs=1.0, k_f=3.0, helicity=cfg["sigma"])
         nzl = rk.slab.nzl
         local = np.empty((7, nzl, n, n), dtype=npdt)
         for q, field in enumerate(inputs.solenoidal_state_fields(n, cfg["seed"])):
@@ -419,7 +420,7 @@ def run_slab(args):
                             "kernel": "substep (per rank; inner + outer launches, halo pack / unpack and ghost kernels "
                                       "charged to it)",
                             "algorithmic_bytes_per_launch": alg}}
-        rk.slab.ctx.ac_free()
+        rk.free()
         del rk, local
         torch.cuda.empty_cache()
         return res
@@ -435,9 +436,11 @@ def run_slab(args):
             "config": {"workload": cfg["name"] + (" x%d along z (weak)" % world if args.weak else ""),
                        "grid": [n, n, nz_global], "nu": nu, "eta": nu, "helicity": cfg["sigma"], "k_f": 3, "f0": 0.02,
                        "dt": main_res["dt"], "variant": args.variant,
-                       "parallelism": "z slabs x%d; halo of 3 planes per side and field per substep, %s" % (
-                           world, "exchanged on a second stream beside the inner-domain update (PAPER.md:141-158)"
-                           if not args.no_overlap else "exchanged before the substep (no overlap)"),
+                       "parallelism": "z slabs x%d; halo of 3 planes per side and field per substep, %s, %s" % (
+                           world, "pulled from the neighbours' memory by one kernel (CUDA IPC / peer memory)"
+                           if args.transport == "pull" else "packed, sent through NCCL, unpacked",
+                           "on a second stream beside the inner-domain update (PAPER.md:141-158)"
+                           if not args.no_overlap else "before the substep (no overlap)"),
                        "l2": "state far larger than L2; no flush needed",
                        "halo_bytes_per_rank_per_substep": main_res["halo_bytes"]},
             "roofline": main_res["roofline"], "cpu_baseline": None, "e2e": None, "gpu_launches": main_res["launches"],
@@ -480,6 +483,9 @@ def main():
     ap.add_argument("--replicas", action="store_true", help="N > 1: N independent boxes instead of one box in z slabs")
     ap.add_argument("--weak", action="store_true", help="slab run with n^2 x n cells per rank (weak scaling, PAPER.md:533)")
     ap.add_argument("--no-overlap", action="store_true", help="slab run: exchange before the substep instead of beside it")
+    ap.add_argument("--transport", default="nccl", choices=["nccl", "pull"],
+                    help="slab run: halo through NCCL send / receive of packed buffers, or pulled from the neighbours' "
+                         "memory by one kernel (CUDA IPC mappings: peer memory over NVLink)")
     ap.add_argument("--paper-protocol", action="store_true",
                     help="the paper's benchmark set-up (PAPER.md:533): all fields U[0,1), no forcing, dt = 1.19209e-7")
     args = ap.parse_args()

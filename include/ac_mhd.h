@@ -172,6 +172,23 @@ size_t ac_halo_bytes(const ac_ctx* ctx);
 int ac_halo_pack(ac_ctx* ctx, void* send_lo_dev, void* send_hi_dev, void* cuda_stream);
 int ac_halo_unpack(ac_ctx* ctx, const void* recv_lo_dev, const void* recv_hi_dev, void* cuda_stream);
 int ac_diag_combine(const ac_ctx* ctx, const double* raws, int nranks, ac_diag* out);
+
+/* The exchange as one kernel over peer memory (no staging buffers, no library collective on the data path):
+ * ac_halo_pull copies the top 3 cell planes of the slab below and the bottom 3 of the slab above straight from THEIR
+ * state arrays into this context's z ghost planes (all fields, x / y ghost zones included, packed fp32 lanes picked),
+ * on cuda_stream (NULL: the context's).  below_workspace / above_workspace = the base of the neighbours' workspaces as
+ * THIS process can address them: ac_workspace_ptr of a context of the same process, or the pointer ac_ipc_open
+ * returns for a handle another process exported with ac_ipc_export (CUDA IPC: the same GPU, or a peer GPU over
+ * NVLink).  All ranks must have the same local grid, dtype and variant and make the same calls in the same order
+ * (the neighbours' current state is then at the same workspace offset as ours).  The caller orders the pull after the
+ * neighbours' previous substep has finished (events; cudaIpcEventHandle between processes) and before its own
+ * AC_PART_OUTER.  ac_ipc_export needs a workspace the library allocated itself (ac_init with workspace_dev = NULL);
+ * the handle is 64 bytes (cudaIpcMemHandle_t).  Errors: AC_EINVAL, AC_ESTATE, AC_ECUDA. */
+int ac_halo_pull(ac_ctx* ctx, const void* below_workspace, const void* above_workspace, void* cuda_stream);
+void* ac_workspace_ptr(ac_ctx* ctx);
+int ac_ipc_export(ac_ctx* ctx, void* handle64);
+int ac_ipc_open(const void* handle64, void** workspace_out);
+int ac_ipc_close(void* workspace);
 int ac_state_layout(const ac_ctx* ctx, ac_layout_info* out);
 void* ac_field_device_ptr(ac_ctx* ctx, int q);
 int ac_reduce_raw(ac_ctx* ctx, double out[6]);

@@ -21,7 +21,8 @@ EXPORTS = (
     "ac_forcing_from_draws", "ac_forcing_params", "ac_make_forcing", "ac_set_bext", "ac_set_cfl", "ac_set_variant",
     "ac_set_upwind", "ac_set_mixed", "ac_substep", "ac_state_layout", "ac_field_device_ptr", "ac_reduce_raw",
     "ac_reduce_ext", "ac_reduce_ext_raw", "ac_set_slab", "ac_substep_part", "ac_halo_bytes", "ac_halo_pack",
-    "ac_halo_unpack", "ac_diag_combine", "ac_set_forcing_mode",
+    "ac_halo_unpack", "ac_diag_combine", "ac_set_forcing_mode", "ac_halo_pull", "ac_workspace_ptr", "ac_ipc_export",
+    "ac_ipc_open", "ac_ipc_close",
     "ac_launch_count", "ac_free", "ac_strerror", "ac_version",
 )
 
@@ -121,6 +122,16 @@ def load_library():
     L.ac_reduce_ext.restype = i32
     L.ac_reduce_ext_raw.argtypes = [vp, ctypes.POINTER(dbl)]
     L.ac_reduce_ext_raw.restype = i32
+    L.ac_halo_pull.argtypes = [vp, vp, vp, vp]
+    L.ac_halo_pull.restype = i32
+    L.ac_workspace_ptr.argtypes = [vp]
+    L.ac_workspace_ptr.restype = ctypes.c_void_p
+    L.ac_ipc_export.argtypes = [vp, vp]
+    L.ac_ipc_export.restype = i32
+    L.ac_ipc_open.argtypes = [vp, ctypes.POINTER(vp)]
+    L.ac_ipc_open.restype = i32
+    L.ac_ipc_close.argtypes = [vp]
+    L.ac_ipc_close.restype = i32
     L.ac_set_forcing_mode.argtypes = [vp, i32]
     L.ac_set_forcing_mode.restype = i32
     L.ac_set_slab.argtypes = [vp, i32, i32]
@@ -174,6 +185,17 @@ def ac_forcing_params(k_f, helicity, cs, shape, lengths, u1, u2, u3, dt, f0):
     return f
 
 
+def ac_ipc_open(handle):
+    """Maps a workspace another process exported with Context.ac_ipc_export; returns its device address here."""
+    out = ctypes.c_void_p()
+    _check(load_library().ac_ipc_open(ctypes.c_char_p(handle), ctypes.byref(out)), "ac_ipc_open")
+    return int(out.value)
+
+
+def ac_ipc_close(ptr):
+    _check(load_library().ac_ipc_close(ctypes.c_void_p(ptr)), "ac_ipc_close")
+
+
 def ac_version():
     return load_library().ac_version().decode()
 
@@ -182,7 +204,7 @@ class Context:
     """One ac_ctx.  Methods carry the C names: ac_load_state, ac_step, ac_reduce, ..."""
 
     def __init__(self, shape, lengths=(2 * np.pi,) * 3, dtype=AC_F64, nu=0.0, eta=0.0, cs=1.0, k_f=3.0,
-                 helicity=0.0, stream=None, device="cuda:0"):
+                 helicity=0.0, stream=None, device="cuda:0", own_workspace=False):
         import torch          # device memory and streams only
         L = load_library()
         if not torch.cuda.is_available():
@@ -198,9 +220,10 @@ class Context:
         if nbytes == 0:
             raise AcError("invalid grid %r" % (self.shape,))
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            # own_workspace: the library cudaMallocs the workspace itself (needed for ac_ipc_export)
+            self.workspace = None if own_workspace else torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        base = self.workspace.data_ptr()
+        base = self.workspace.data_ptr() if self.workspace is not None else 0
         aligned = (base + 255) // 256 * 256
         self._ctx = ctypes.c_void_p()
         with torch.cuda.device(self.device):       # the library records the current device as the context's
@@ -305,6 +328,19 @@ class Context:
     def ac_halo_unpack(self, recv_lo, recv_hi, stream=None):
         _check(self._lib.ac_halo_unpack(self._ctx, ctypes.c_void_p(recv_lo.data_ptr()), ctypes.c_void_p(recv_hi.data_ptr()),
                                         ctypes.c_void_p(stream.cuda_stream if stream is not None else 0)), "ac_halo_unpack")
+
+    def ac_halo_pull(self, below_workspace, above_workspace, stream=None):
+        """below_workspace / above_workspace: integer device addresses (ac_workspace_ptr or ac_ipc_open)."""
+        _check(self._lib.ac_halo_pull(self._ctx, ctypes.c_void_p(below_workspace), ctypes.c_void_p(above_workspace),
+                                      ctypes.c_void_p(stream.cuda_stream if stream is not None else 0)), "ac_halo_pull")
+
+    def ac_workspace_ptr(self):
+        return int(self._lib.ac_workspace_ptr(self._ctx))
+
+    def ac_ipc_export(self):
+        buf = ctypes.create_string_buffer(64)
+        _check(self._lib.ac_ipc_export(self._ctx, buf), "ac_ipc_export")
+        return buf.raw
 
     def ac_diag_combine(self, raws):
         """raws: sequence of ac_reduce_raw tuples, one per rank, in rank order."""

@@ -915,6 +915,58 @@ int ac_halo_unpack(ac_ctx* ctx, const void* recv_lo_dev, const void* recv_hi_dev
     return AC_OK;
 }
 
+int ac_halo_pull(ac_ctx* ctx, const void* below_workspace, const void* above_workspace, void* cuda_stream) {
+    DeviceGuard guard(ctx);
+    if (!ctx || !below_workspace || !above_workspace) return AC_EINVAL;
+    if (!ctx->loaded) return AC_ESTATE;
+    cudaStream_t st = cuda_stream ? (cudaStream_t)cuda_stream : ctx->stream;
+    const ac::Layout& L = ctx->L;
+    const size_t per_field = (size_t)ac::R * L.plane;
+    dim3 grd((unsigned)((per_field + 255) / 256), AC_NFIELDS, 1);
+    // every rank of a run makes the same calls in the same order, so the neighbours' current state sits at the same
+    // offset of their workspace as ours does in ours
+    const size_t off = (size_t)((char*)ctx->field_ptr(ctx->cur, 0) - ctx->ws);
+    void* state = ctx->field_ptr(ctx->cur, 0);
+    const void* below = (const char*)below_workspace + off;
+    const void* above = (const char*)above_workspace + off;
+    if (ctx->dtype == AC_F64)
+        ac::halo_pull_kernel<double, 1><<<grd, 256, 0, st>>>(state, below, above, L.field, L);
+    else if (ctx->packed)
+        ac::halo_pull_kernel<float, 2><<<grd, 256, 0, st>>>(state, below, above, L.field, L);
+    else
+        ac::halo_pull_kernel<float, 1><<<grd, 256, 0, st>>>(state, below, above, L.field, L);
+    ctx->launches++;
+    AC_CUDA(cudaGetLastError());
+    return AC_OK;
+}
+
+void* ac_workspace_ptr(ac_ctx* ctx) { return ctx ? (void*)ctx->ws : nullptr; }
+
+int ac_ipc_export(ac_ctx* ctx, void* handle64) {
+    DeviceGuard guard(ctx);
+    if (!ctx || !handle64) return AC_EINVAL;
+    if (!ctx->owns_ws) return AC_ESTATE;       // only a workspace the library allocated starts at a cudaMalloc base
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "the header promises a 64-byte handle");
+    cudaIpcMemHandle_t h;
+    AC_CUDA(cudaIpcGetMemHandle(&h, ctx->ws));
+    memcpy(handle64, &h, 64);
+    return AC_OK;
+}
+
+int ac_ipc_open(const void* handle64, void** workspace_out) {
+    if (!handle64 || !workspace_out) return AC_EINVAL;
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle64, 64);
+    AC_CUDA(cudaIpcOpenMemHandle(workspace_out, h, cudaIpcMemLazyEnablePeerAccess));
+    return AC_OK;
+}
+
+int ac_ipc_close(void* workspace) {
+    if (!workspace) return AC_EINVAL;
+    AC_CUDA(cudaIpcCloseMemHandle(workspace));
+    return AC_OK;
+}
+
 int ac_diag_combine(const ac_ctx* ctx, const double* raws, int nranks, ac_diag* out) {
     if (!ctx || !raws || !out || nranks < 1) return AC_EINVAL;
     double su = 0.0, sb = 0.0, mu = 0.0, mb = 0.0, lmin = INFINITY, lmax = -INFINITY;

@@ -95,6 +95,24 @@ __global__ void halo_unpack_kernel(void* __restrict__ state, size_t field_elems,
     f[((size_t)(L.nz + R) * L.plane + i) * LANES + (LANES - 1)] = hi[q * per_field + i];  // ghost planes above
 }
 
+// The same exchange as ONE kernel over peer memory: the ghost planes are pulled straight from the neighbours' state
+// arrays (device pointers of the same GPU, or peer-mapped pointers of another GPU: NVLink loads), no staging buffers,
+// no library collective.  below / above = the neighbours' buffers that hold THEIR current state, same layout as ours.
+template <typename T, int LANES>
+__global__ void halo_pull_kernel(void* __restrict__ state, const void* __restrict__ below, const void* __restrict__ above,
+                                 size_t field_elems, Layout L) {
+    const size_t per_field = (size_t)R * L.plane;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= per_field) return;
+    const int q = blockIdx.y;
+    T* f = (T*)state + (size_t)q * field_elems * LANES;
+    const T* fb = (const T*)below + (size_t)q * field_elems * LANES;
+    const T* fa = (const T*)above + (size_t)q * field_elems * LANES;
+    // ghost planes below <- the top cell planes of the slab below; ghost planes above <- the bottom cell planes of the one above
+    f[i * LANES] = fb[((size_t)L.nz * L.plane + i) * LANES + (LANES - 1)];
+    f[((size_t)(L.nz + R) * L.plane + i) * LANES + (LANES - 1)] = fa[((size_t)R * L.plane + i) * LANES];
+}
+
 // ------------------------------------------------------------------------------------------------
 // forcing tables (S7): cos/sin of k_a x_a per axis, phase folded into the z table.
 // layout: [cx(nx) sx(nx) cy(ny) sy(ny) cz(nz) sz(nz)]

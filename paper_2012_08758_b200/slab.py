@@ -7,7 +7,10 @@ Every rank owns nz / p planes and runs the ordinary context on them.  A substep 
 WHILE the inner planes are updated on the compute stream; the 3 + 3 boundary planes follow once the halo has landed.
 Transport: torch.distributed point-to-point operations on the dense halo buffers (NCCL between GPUs; gloo with host
 staging for the multi-process test on one GPU), or device-to-device copies for several slabs held by one process (the
-one-GPU emulation).  No kernel waits on another rank.
+one-GPU emulation).  transport="pull" replaces pack / send / receive / unpack by ONE kernel that reads the neighbours'
+boundary planes straight from their state arrays (ac_halo_pull): device pointers inside a process, CUDA IPC mappings
+between processes (peer memory over NVLink between GPUs), ordered by events (interprocess events between processes,
+whose record / wait calls a host barrier keeps in sequence).  No kernel waits on another rank.
 """
 import numpy as np
 
@@ -42,7 +45,8 @@ class _HostStream:
 class Slab:
     """One rank's context, its halo buffers and its two streams."""
 
-    def __init__(self, global_shape, lengths, rank, world, dtype=binding.AC_F64, variant=0, context_factory=None, **kw):
+    def __init__(self, global_shape, lengths, rank, world, dtype=binding.AC_F64, variant=0, context_factory=None,
+                 interprocess=False, **kw):
         import torch
         nz, ny, nx = global_shape
         if nz % world != 0 or nz // world < 8:
@@ -59,7 +63,7 @@ class Slab:
         if torch.device(dev).type == "cuda":
             with torch.cuda.device(dev):
                 self.comm = torch.cuda.Stream(device=dev)
-            self.state_ready = torch.cuda.Event()
+            self.state_ready = torch.cuda.Event(interprocess=True) if interprocess else torch.cuda.Event()
             self.halo_ready = torch.cuda.Event()
         else:
             self.comm = self.state_ready = self.halo_ready = _HostStream()
@@ -78,6 +82,19 @@ class Slab:
 
     def wait_halo(self):
         self.ctx.stream.wait_event(self.halo_ready)
+
+    # the exchange as one kernel over the neighbours' memory
+    def mark_state(self):
+        self.state_ready.record(self.ctx.stream)
+
+    def pull(self, below_ws, above_ws, below_ready, above_ready):
+        """below_ws / above_ws: addresses of the neighbours' workspaces; *_ready: their state_ready events."""
+        self.comm.wait_event(self.state_ready)
+        self.comm.wait_event(below_ready)
+        self.comm.wait_event(above_ready)
+        self.ctx.ac_halo_pull(below_ws, above_ws, self.comm)
+        self.halo_ready.record(self.comm)
+        self.halo_valid = True
 
 
 def transfer_in_process(slabs):
@@ -142,16 +159,33 @@ class SlabGroupInProcess:
     """p slabs of one box driven by one process on one GPU: the reference behaviour of the decomposition."""
 
     def __init__(self, global_shape, lengths, world, dtype=binding.AC_F64, variant=0, overlap=True, context_factory=None,
-                 **kw):
+                 transport="buffers", **kw):
         self.shape, self.lengths, self.kw, self.overlap = tuple(global_shape), tuple(lengths), kw, overlap
+        self.transport = transport
         self.slabs = [Slab(global_shape, lengths, r, world, dtype, variant, context_factory, **kw) for r in range(world)]
 
+    def exchange_begin(self):
+        if self.transport == "pull":
+            for s in self.slabs:
+                s.mark_state()
+        else:
+            for s in self.slabs:
+                s.pack()
+
+    def exchange_end(self):
+        p = len(self.slabs)
+        if self.transport == "pull":
+            for r, s in enumerate(self.slabs):
+                below, above = self.slabs[(r - 1) % p], self.slabs[(r + 1) % p]
+                s.pull(below.ctx.ac_workspace_ptr(), above.ctx.ac_workspace_ptr(), below.state_ready, above.state_ready)
+        else:
+            transfer_in_process(self.slabs)
+            for s in self.slabs:
+                s.unpack()
+
     def exchange(self):
-        for s in self.slabs:
-            s.pack()
-        transfer_in_process(self.slabs)
-        for s in self.slabs:
-            s.unpack()
+        self.exchange_begin()
+        self.exchange_end()
 
     def load_state(self, state):
         nzl = self.slabs[0].nzl
@@ -162,13 +196,12 @@ class SlabGroupInProcess:
     def step(self, dt, forcing=None):
         """forcing: of the GLOBAL box (every slab shifts the phase itself)."""
         for sub in range(3):
-            for s in self.slabs:
-                s.pack()                                      # communication stream, after the previous substep
-                if self.overlap:
+            self.exchange_begin()                             # communication stream, after the previous substep
+            if self.overlap:
+                for s in self.slabs:
                     s.ctx.ac_substep_part(sub, dt, forcing, binding.AC_PART_INNER)    # runs beside the exchange
-            transfer_in_process(self.slabs)
+            self.exchange_end()
             for s in self.slabs:
-                s.unpack()
                 s.wait_halo()
                 if self.overlap:
                     s.ctx.ac_substep_part(sub, dt, forcing, binding.AC_PART_OUTER)
@@ -198,10 +231,39 @@ class SlabRank:
     """One process per rank (torchrun): this rank's slab of the box, exchanged through torch.distributed."""
 
     def __init__(self, global_shape, lengths, dist, dtype=binding.AC_F64, device="cuda:0", variant=0, overlap=True,
-                 context_factory=None, **kw):
+                 context_factory=None, transport="buffers", **kw):
         self.dist, self.rank, self.world = dist, dist.get_rank(), dist.get_world_size()
         self.shape, self.lengths, self.kw, self.overlap = tuple(global_shape), tuple(lengths), kw, overlap
-        self.slab = Slab(global_shape, lengths, self.rank, self.world, dtype, variant, context_factory, device=device, **kw)
+        self.transport = transport
+        if transport == "pull":
+            kw = dict(kw, own_workspace=True)                 # ac_ipc_export needs a workspace the library allocated
+        self.slab = Slab(global_shape, lengths, self.rank, self.world, dtype, variant, context_factory,
+                         interprocess=transport == "pull", device=device, **kw)
+        if transport == "pull":
+            self._open_neighbours()
+
+    def _open_neighbours(self):
+        """CUDA IPC: map the neighbours' workspaces and import their state_ready events."""
+        import torch
+        s, dist = self.slab, self.dist
+        self.host_group = dist.new_group(backend="gloo") if dist.get_backend() != "gloo" else None
+        mine = (s.ctx.ac_ipc_export(), s.state_ready.ipc_handle())
+        everyone = [None] * self.world
+        dist.all_gather_object(everyone, mine, group=self.host_group)
+        self._opened = {}
+        self.nb_ws, self.nb_ready = [], []
+        for r in ((self.rank - 1) % self.world, (self.rank + 1) % self.world):
+            if r == self.rank:
+                self.nb_ws.append(s.ctx.ac_workspace_ptr())
+                self.nb_ready.append(s.state_ready)
+                continue
+            if r not in self._opened:
+                ws = binding.ac_ipc_open(everyone[r][0])
+                ev = torch.cuda.Event.from_ipc_handle(torch.device(s.ctx.device), everyone[r][1])
+                self._opened[r] = (ws, ev)
+            self.nb_ws.append(self._opened[r][0])
+            self.nb_ready.append(self._opened[r][1])
+
 
     def forcing_from_draws(self, u1, u2, u3, dt, f0):
         """Eq. 4-6 for the GLOBAL box (a slab context knows the global box, ac_set_slab)."""
@@ -215,10 +277,38 @@ class SlabRank:
         else:
             transfer_in_process([self.slab])
 
+    def exchange_begin(self):
+        if self.transport == "pull":
+            self.slab.mark_state()
+        else:
+            self.slab.pack()
+
+    def exchange_end(self):
+        if self.transport == "pull":
+            # every rank has issued its record before any rank issues the wait on it (a host barrier: no device sync)
+            if self.world > 1:
+                self.dist.barrier(group=self.host_group)
+            self.slab.pull(self.nb_ws[0], self.nb_ws[1], self.nb_ready[0], self.nb_ready[1])
+        else:
+            self.transfer()
+            self.slab.unpack()
+
     def exchange(self):
-        self.slab.pack()
-        self.transfer()
-        self.slab.unpack()
+        self.exchange_begin()
+        self.exchange_end()
+
+    def free(self):
+        if self.transport == "pull":
+            self.slab.ctx.synchronize()
+            self.slab.comm.synchronize()
+            if self.world > 1:
+                self.dist.barrier(group=self.host_group)     # nobody unmaps memory a neighbour still reads
+            for ws, _ in self._opened.values():
+                binding.ac_ipc_close(ws)
+            self._opened = {}
+            if self.world > 1:
+                self.dist.barrier(group=self.host_group)
+        self.slab.ctx.ac_free()
 
     def load_state(self, state):
         """state: the GLOBAL (7, nz, ny, nx) array (every rank generates the same seeded input) or this rank's slab."""
@@ -231,11 +321,10 @@ class SlabRank:
     def step(self, dt, forcing=None):
         s = self.slab
         for sub in range(3):
-            s.pack()                                          # communication stream, after the previous substep
+            self.exchange_begin()                             # communication stream, after the previous substep
             if self.overlap:
                 s.ctx.ac_substep_part(sub, dt, forcing, binding.AC_PART_INNER)        # runs beside the exchange
-            self.transfer()
-            s.unpack()
+            self.exchange_end()
             s.wait_halo()
             if self.overlap:
                 s.ctx.ac_substep_part(sub, dt, forcing, binding.AC_PART_OUTER)

@@ -17,6 +17,7 @@ from paper_2012_08758_b200 import binding, inputs, slab  # noqa: E402
 def main():
     out_dir = sys.argv[1]
     backend = sys.argv[2] if len(sys.argv) > 2 else "gloo"
+    transport = sys.argv[3] if len(sys.argv) > 3 else "buffers"
     if backend == "nccl":
         import torch
         torch.cuda.set_device(0)
@@ -26,7 +27,8 @@ def main():
     shape = (32, 24, 32)
     lengths = (2 * math.pi, 1.5 * math.pi, 3.0 * math.pi)
     state = inputs.smooth_strong_state(shape, 41)
-    rk = slab.SlabRank(shape, lengths, dist, binding.AC_F64, nu=5e-3, eta=4e-3, cs=1.0, k_f=3, helicity=1.0)
+    rk = slab.SlabRank(shape, lengths, dist, binding.AC_F64, transport=transport, nu=5e-3, eta=4e-3, cs=1.0, k_f=3,
+                       helicity=1.0)
     rk.load_state(state)
     dt = 2e-3
     for s in range(2):
@@ -37,6 +39,7 @@ def main():
     if rk.rank == 0:
         np.save(os.path.join(out_dir, "diag.npy"), np.array([d["urms"], d["brms"], d["umax"], d["bmax"], d["dt_cfl"]]))
     dist.barrier()
+    rk.free()
     dist.destroy_process_group()
 
 

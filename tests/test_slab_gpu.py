@@ -141,3 +141,56 @@ def test_slab_rank_over_nccl_with_one_rank(tmp_path):
     assert np.array_equal(got, want)
     for v, key in zip(diag, ("urms", "brms", "umax", "bmax", "dt_cfl")):
         assert abs(v - d[key]) <= 1e-13 * abs(d[key]), key
+
+
+@pytest.mark.parametrize("dtype", [binding.AC_F64, binding.AC_F32])
+@pytest.mark.parametrize("world", [2, 3])
+def test_slabs_with_the_pull_kernel_equal_single_context(world, dtype):
+    """transport="pull": the ghost planes come straight out of the neighbours' state arrays (ac_halo_pull, one kernel,
+    no staging buffers), here between contexts of one process; packed fp32 lanes included."""
+    shape = (48, 24, 32)
+    lengths = (2 * math.pi, 1.5 * math.pi, 3.0 * math.pi)
+    npdt = np.float64 if dtype == binding.AC_F64 else np.float32
+    state = inputs.smooth_strong_state(shape, 43).astype(npdt)
+    kw = dict(nu=5e-3, eta=4e-3, cs=1.0, k_f=3, helicity=0.5)
+    one = binding.Context(shape, lengths, dtype, **kw)
+    grp = slab.SlabGroupInProcess(shape, lengths, world, dtype, transport="pull", **kw)
+    one.ac_load_state(state)
+    grp.load_state(state)
+    dt = 2e-3
+    for _ in range(3):
+        one.ac_step(dt, None)
+        grp.step(dt, None)
+    assert np.array_equal(one.ac_store_state(), grp.store_state())
+    d1, dg = one.ac_reduce(), grp.reduce()
+    for key in ("urms", "umax", "brms", "bmax", "dt_cfl"):
+        assert abs(d1[key] - dg[key]) <= 1e-13 * abs(d1[key]), key
+    one.ac_free()
+    grp.free()
+
+
+def test_slab_ranks_pull_over_cuda_ipc(tmp_path):
+    """Two ranks as separate processes whose pull kernels read each other's workspace through CUDA IPC mappings,
+    ordered by interprocess events (both processes share the one GPU here; between GPUs the same mappings are peer
+    memory over NVLink).  No kernel waits on another rank: the ordering is stream waits on events."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+           "127.0.0.1", "--master-port", "29555", os.path.join(root, "tests", "slab_worker.py"), str(tmp_path), "gloo",
+           "pull"]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=root)
+    assert r.returncode == 0, r.stderr[-3000:]
+    got = np.concatenate([np.load(tmp_path / ("slab_%d.npy" % k)) for k in range(2)], axis=1)
+    shape = (32, 24, 32)
+    lengths = (2 * math.pi, 1.5 * math.pi, 3.0 * math.pi)
+    one = binding.Context(shape, lengths, binding.AC_F64, nu=5e-3, eta=4e-3, cs=1.0, k_f=3, helicity=1.0)
+    one.ac_load_state(inputs.smooth_strong_state(shape, 41))
+    dt = 2e-3
+    for s in range(2):
+        one.ac_step(dt, one.ac_forcing_from_draws(0.3 + 0.1 * s, 0.6, 0.2, dt, 0.02))
+    err = helpers.max_group_error(got, one.ac_store_state())
+    one.ac_free()
+    print("2 processes, pull over CUDA IPC:", err)
+    assert err <= 1e-13
