@@ -21,7 +21,9 @@
 //    TENSOR MEMORY (tcgen05.st when a plane arrives, tcgen05.ld three planes later): a per-lane scratchpad
 //    that costs no shared-memory bandwidth.  The in-plane first derivatives that wait three planes for
 //    their z partners are parked there too, and so is the (j x B)/rho mailbox: U warp w and A warp w + 4
-//    address the same 32 tensor-memory lanes, so A lane i writes what U lane i reads.
+//    address the same 32 tensor-memory lanes, so A lane i writes what U lane i reads.  The forcing f of Eq. 4
+//    rides on the mailbox ((j x B)/rho + f): the step time follows the longer of the two roles, and the A role
+//    had the slack.
 // 3. The level shift of the accumulators is folded into the scatter (new[r-1] = old[r] + w v): no
 //    register moves in the loop.
 //
