@@ -162,3 +162,33 @@ def test_config3_256cubed_ten_steps_fp64():
     err = helpers.group_errors(got, st.state)
     print("256^3, 10 steps, fp64:", err)
     assert max(err.values()) <= 1e-9
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("dtype", [binding.AC_F64, binding.AC_F32])
+def test_degenerate_states_are_fixed_points(variant, dtype):
+    """Degenerate cases of the method: a uniform state (constant ln rho, u, A; no forcing) has an exactly vanishing
+    right-hand side - every stencil sums differences of equal numbers - so the step must return it BITWISE, with
+    viscosity and resistivity on, on a ragged grid; and with A = 0 the magnetic part stays exactly zero while the
+    hydrodynamic part moves."""
+    shape = (24, 9, 40)
+    lengths = (2 * math.pi, 1.3 * math.pi, 2.9 * math.pi)
+    npdt = np.float64 if dtype == binding.AC_F64 else np.float32
+    ctx = binding.Context(shape, lengths, dtype, nu=1e-2, eta=2e-2, cs=1.3)
+    ctx.ac_set_variant(variant)
+    state = np.empty((7,) + shape, dtype=npdt)
+    for q, v in enumerate((0.3, 0.2, -0.1, 0.05, 1e-3, -2e-3, 3e-3)):
+        state[q] = v
+    ctx.ac_load_state(state)
+    for _ in range(3):
+        ctx.ac_step(1e-3, None)
+    assert np.array_equal(ctx.ac_store_state(), state)
+    d = ctx.ac_reduce()
+    assert d["brms"] == 0.0 and d["bmax"] == 0.0 and d["lnrho_min"] == d["lnrho_max"] == float(npdt(0.3))
+    moving = inputs.smooth_strong_state(shape, 7).astype(npdt)
+    moving[4:7] = 0.0
+    ctx.ac_load_state(moving)
+    ctx.ac_step(1e-3, None)
+    out = ctx.ac_store_state()
+    ctx.ac_free()
+    assert np.all(out[4:7] == 0.0) and not np.array_equal(out[1:4], moving[1:4])
