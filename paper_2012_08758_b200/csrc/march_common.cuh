@@ -13,7 +13,7 @@ namespace ac {
 constexpr int M_TX = 16, M_TY = 8, M_COLS = M_TX * M_TY;
 constexpr int M_WORKERS = 2 * M_COLS;          // U and A roles
 constexpr int M_THREADS = M_WORKERS + 128;    // + the producer warpgroup (one working lane) that feeds the ring
-constexpr int M_REGS_WORKER = 232, M_REGS_PRODUCER = 40;   // setmaxnreg: 128 x (232 + 232 + 40) = 384 x 168, the registers the CTA is launched with
+constexpr int M_REGS_WORKER = 240, M_REGS_PRODUCER = 24;   // setmaxnreg: 128 x (240 + 240 + 24) = 384 x 168, the registers the CTA is launched with
 constexpr int M_HX = 4;                  // x halo of the tile in shared memory (>= R; 32 bytes keeps TMA boxes aligned)
 constexpr int M_WX = M_TX + 2 * M_HX;    // 24
 constexpr int M_WY = M_TY + 2 * R;       // 14
