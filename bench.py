@@ -184,6 +184,7 @@ def run_ours(args):
         ctx = binding.Context((n, n, n), TWO_PI3, dtype, nu=nu, eta=nu, cs=1.0, k_f=3.0, helicity=cfg["sigma"],
                               device="cuda:%d" % local_rank)
         ctx.ac_set_variant(args.variant)
+        ctx.ac_set_mixed(args.mixed)
         # pinned host copy of the state, filled field by field (1024^3 fp64: 60 GB, 8.6 GB per field)
         host = torch.empty((7, n, n, n), dtype=torch.float64 if dtype_name == "f64" else torch.float32, pin_memory=True)
         hview = host.numpy()
@@ -330,6 +331,7 @@ def run_ours(args):
             "config": {"workload": cfg["name"], "grid": [n, n, n], "nu": nu, "eta": nu, "helicity": cfg["sigma"],
                        "k_f": 3, "f0": 0.02, "dt": main["dt"], "l2": "state (14 arrays) far larger than L2; no flush needed",
                        "parallelism": "replicas only" if world > 1 else "single GPU", "variant": args.variant,
+                       "mixed": args.mixed,
                        "protocol": "paper (PAPER.md:533)" if args.paper_protocol else "baseline"},
             "ms_median": main["ms_median"], "ms_p90": main["ms_p90"],
             "roofline": main["roofline"], "cpu_baseline": cpu, "e2e": main.get("e2e"),
@@ -473,6 +475,8 @@ def main():
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--n", type=int, default=512)
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--mixed", default="bidiagonal", choices=["bidiagonal", "tensor"],
+                    help="reading of the mixed-derivative scheme (G2); every BASELINE number uses bidiagonal")
     ap.add_argument("--single-dtype", action="store_true", help="skip the second precision")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--quick-cpu", action="store_true", help="cpu_baseline without the 256^3 box")

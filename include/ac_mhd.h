@@ -246,8 +246,11 @@ int ac_set_upwind(ac_ctx* ctx, int on);
 int ac_set_forcing_mode(ac_ctx* ctx, int mode);
 /* ac_set_mixed: reading of the mixed-derivative scheme, which the paper does not print (G2).  0 (default, all
  * reported parity and every BASELINE config) = bidiagonal 12-point stencil; 1 = tensor product D_a(D_b f), 36
- * points, also radius 3 and 6th order.  Mode 1 runs the direct kernel whatever the variant.  Like ac_set_variant
- * it must be called before ac_load_state (a loaded state is dropped: AC_ESTATE until the next load). */
+ * points, also radius 3 and 6th order, taken as D_z (D_x f), D_z (D_y f), D_y (D_x f).  With the default kernel
+ * (variant 0) mode 1 is a build of the same fused substep kernel in which the z-mixed terms are z stencils of the
+ * in-plane first derivatives and the in-plane ones are y stencils of d_x f staged in shared memory (SURVEY.md 8(f)
+ * NEXT-4, "staged intermediates"); variants 1 and 2 run the direct kernel.  Like ac_set_variant it must be called
+ * before ac_load_state (a loaded state is dropped: AC_ESTATE until the next load). */
 int ac_set_mixed(ac_ctx* ctx, int mode);
 int ac_set_cfl(ac_ctx* ctx, double c_u, double c_nu);
 int ac_set_variant(ac_ctx* ctx, int variant);

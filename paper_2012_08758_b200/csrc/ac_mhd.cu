@@ -145,7 +145,7 @@ struct ac_ctx {
     double c_u, c_nu;
     int upwind;          // 1 = upwinded continuity equation (G17); default 0
     int forcing_kick;    // 1 = alternative reading of G8: one impulse u += dt f per step, applied with substep 2; default 0
-    int mixed;           // 0 = bidiagonal mixed stencil (G2, default), 1 = tensor product (direct kernel only)
+    int mixed;           // 0 = bidiagonal mixed stencil (G2, default), 1 = tensor product (pair-march MIX build, direct kernel)
     int variant;         // requested: 0 = pair-march (default), 1 = direct, 2 = scatter-march (one cell per thread)
     bool march;          // the kernel actually used (fp32 with odd nz falls back to direct)
     bool packed;         // fp32 cells stored as (z, z + nz/2) pairs
@@ -268,6 +268,9 @@ void fill_march_coef(const ac_ctx* ctx, ac::MarchCoef<E>& c, double dt, int s, c
         c.c1y[m] = S::of(c1[1][m]);
         c.c1z[m] = S::of(c1[2][m]);
         c.nc1z[m] = S::of(-c1[2][m]);
+        c.c13y[m] = S::of(c1[1][m] / 3.0);
+        c.c13z[m] = S::of(c1[2][m] / 3.0);
+        c.nc13z[m] = S::of(-c1[2][m] / 3.0);
         const double mxy = WM[m] / (h[0] * h[1]), mxz = WM[m] / (h[0] * h[2]), myz = WM[m] / (h[1] * h[2]);
         c.cm3xy[m] = S::of(mxy / 3.0);
         c.cm3xz[m] = S::of(mxz / 3.0);
@@ -392,7 +395,13 @@ int substep_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s, int part
             if (ctx->variant == 0) {
                 // pair-march: 16 x 16 tiles, a thread owns two cells
                 dim3 gq((L.nx + ac::Q_TX - 1) / ac::Q_TX, (L.ny + ac::Q_TY - 1) / ac::Q_TY, nch);
-                if (ctx->upwind)
+                if (ctx->mixed == 1 && ctx->upwind)
+                    ac::substep_pair_kernel<T, true, true><<<gq, ac::Q_THREADS, ac::QX_SMEM_BYTES, ctx->stream>>>(
+                        a, ctx->map_qin[ctx->cur], ctx->map_qprev[1 - ctx->cur]);
+                else if (ctx->mixed == 1)
+                    ac::substep_pair_kernel<T, false, true><<<gq, ac::Q_THREADS, ac::QX_SMEM_BYTES, ctx->stream>>>(
+                        a, ctx->map_qin[ctx->cur], ctx->map_qprev[1 - ctx->cur]);
+                else if (ctx->upwind)
                     ac::substep_pair_kernel<T, true><<<gq, ac::Q_THREADS, ac::Q_SMEM_BYTES, ctx->stream>>>(
                         a, ctx->map_qin[ctx->cur], ctx->map_qprev[1 - ctx->cur]);
                 else
@@ -413,7 +422,8 @@ int substep_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s, int part
             // S1: refresh the ghost zones of the buffer just written.  The z ghost planes of a slab belong to its
             // neighbours (ac_halo_unpack); of packed fp32 pairs one lane is the slab's own cell, so they are kept.
             const int nb_rows = 2 * ac::R * L.my + 2 * ac::R * L.nz;
-            const int na_tasks = (int)(((long)L.ny * L.nz + ac::M_GHOST_ROWS_PER_TASK - 1) / ac::M_GHOST_ROWS_PER_TASK);
+            const int rows_per_task = ac::M_GHOST_THREADS / (2 * L.gx);
+            const int na_tasks = (int)(((long)L.ny * L.nz + rows_per_task - 1) / rows_per_task);
             const int first_row = (ctx->slab && !ctx->packed) ? 2 * ac::R * L.my : 0;
             dim3 gg((unsigned)std::min(nb_rows + na_tasks - first_row, RED_BLOCKS), AC_NFIELDS, 1);
             ac::ghost_fill_kernel<E><<<gg, ac::M_GHOST_THREADS, 0, ctx->stream>>>((E*)ctx->field_ptr(1 - ctx->cur, 0), L,
@@ -608,7 +618,8 @@ namespace {
 // choose the kernel and the device layout for the context's variant; builds the TMA maps
 int configure(ac_ctx* ctx) {
     const ac_grid* g = &ctx->grid;
-    ctx->march = ctx->variant != 1 && ctx->mixed == 0 && (ctx->dtype == AC_F64 || can_pack(g));
+    // the tensor-product reading of the mixed derivatives (NEXT-4) exists in the pair-march and in the direct kernel
+    ctx->march = ctx->variant != 1 && (ctx->mixed == 0 || ctx->variant == 0) && (ctx->dtype == AC_F64 || can_pack(g));
     ctx->packed = ctx->march && ctx->dtype == AC_F32;
     ctx->L = layout_for(g, ctx->dtype, ctx->packed);
     ctx->cv = carve(ctx->L, store_elem_size(ctx->dtype, ctx->packed), elem_size(ctx->dtype), g->nz);
@@ -642,18 +653,22 @@ int configure(ac_ctx* ctx) {
         if (rc == AC_OK) rc = make_state_map(&ctx->map_qprev[b], ctx->field_ptr(b, 0), ctx->L, ac::Q_TX, ac::Q_TY);
         if (rc != AC_OK) return rc;
     }
-    const void* kernels[8] = {(const void*)ac::substep_march_kernel<double, false>,
+    const void* kernels[12] = {(const void*)ac::substep_march_kernel<double, false>,
                               (const void*)ac::substep_march_kernel<double, true>,
                               (const void*)ac::substep_march_kernel<float, false>,
                               (const void*)ac::substep_march_kernel<float, true>,
                               (const void*)ac::substep_pair_kernel<double, false>,
                               (const void*)ac::substep_pair_kernel<double, true>,
                               (const void*)ac::substep_pair_kernel<float, false>,
-                              (const void*)ac::substep_pair_kernel<float, true>};
-    for (int k = 0; k < 8; k++) {
+                              (const void*)ac::substep_pair_kernel<float, true>,
+                              (const void*)ac::substep_pair_kernel<double, false, true>,
+                              (const void*)ac::substep_pair_kernel<double, true, true>,
+                              (const void*)ac::substep_pair_kernel<float, false, true>,
+                              (const void*)ac::substep_pair_kernel<float, true, true>};
+    for (int k = 0; k < 12; k++) {
         if ((ctx->dtype == AC_F64) != (k % 4 < 2)) continue;
         cudaError_t ea = cudaFuncSetAttribute(kernels[k], cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                              k < 4 ? ac::M_SMEM_BYTES : ac::Q_SMEM_BYTES);
+                                              k < 4 ? ac::M_SMEM_BYTES : (k < 8 ? ac::Q_SMEM_BYTES : ac::QX_SMEM_BYTES));
         if (ea != cudaSuccess) return cuda_fail(ea, "cudaFuncSetAttribute(march kernel smem)");
     }
     // z chunks: every chunk re-reads 6 planes, every wave of CTAs costs (planes + 6) iterations;
@@ -1175,7 +1190,7 @@ int ac_set_mixed(ac_ctx* ctx, int mode) {
     DeviceGuard guard(ctx);
     if (!ctx || (mode != 0 && mode != 1)) return AC_EINVAL;
     if (mode == ctx->mixed) return AC_OK;
-    // the tensor-product reading exists in the direct kernel only, whose fp32 device layout differs
+    // variants 1 and 2 run the tensor-product reading in the direct kernel, whose fp32 device layout differs
     cudaStreamSynchronize(ctx->stream);
     ctx->mixed = mode;
     return configure(ctx);

@@ -53,6 +53,8 @@ struct MarchCoef {
     E c6x[3], c6y[3], c6z[3], c60x, c60y, c60z;
     // physics and time stepping
     E nu, eta, ncs2, bext[3], rk_a, rk_b, fre[3], nfim[3], n23;
+    // tensor-product mixed derivatives (pair-march MIX build): 1/3 of the first-derivative weights
+    E c13y[3], c13z[3], nc13z[3];
 };
 
 template <typename T>

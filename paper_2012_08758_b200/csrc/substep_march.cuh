@@ -93,14 +93,16 @@ __device__ __forceinline__ E m_mixxy(const E* p, const E (&cm)[3]) {
 // transfer"; wrap of PAPER.md:111).  Every ghost cell copies its periodic source
 // cell, which is always an interior cell, so the order of the copies does not matter.  Tasks
 // [0, nb_rows) are the rows that are ghosts in y or z (whole rows, x ghosts included), the remaining
-// tasks the 2 x 3 x-ghost cells of 42 interior rows each; blocks take tasks round-robin.  z images of packed fp32
+// tasks the x ghosts of M_GHOST_THREADS / (2 gx) interior rows each; blocks take tasks round-robin.  The x ghosts
+// are copied as whole 32-byte sectors (gx elements a side: the R ghost cells and the alignment pad next to
+// them, which nothing reads), so that no store leaves a partly written sector.  z images of packed fp32
 // pairs swap lanes (cell z - nz/2 of the pair below is cell z + nz/2 of the periodic domain).
 constexpr int M_GHOST_THREADS = 256;
-constexpr int M_GHOST_ROWS_PER_TASK = M_GHOST_THREADS / (2 * R);   // interior rows whose 6 x ghosts one task copies
 template <typename E>
 __global__ void __launch_bounds__(M_GHOST_THREADS) ghost_fill_kernel(E* __restrict__ base, Layout L, int nb_rows, int na_tasks, int first_row) {
     E* __restrict__ f = base + (size_t)blockIdx.y * L.field;
     const int tid = threadIdx.x;
+    const int per_row = 2 * L.gx, rows_per_task = M_GHOST_THREADS / per_row;
     // first_row = 2 R my skips the 6 ghost planes (a slab whose neighbours fill them)
     for (int task = first_row + blockIdx.x; task < nb_rows + na_tasks; task += gridDim.x) {
         if (task < nb_rows) {
@@ -121,20 +123,20 @@ __global__ void __launch_bounds__(M_GHOST_THREADS) ghost_fill_kernel(E* __restri
             const int zs = z < 0 ? z + L.nz : (z >= L.nz ? z - L.nz : z);
             const E* __restrict__ src = f + L.idx(0, ys, zs);
             E* __restrict__ dst = f + L.idx(0, y, z);
-            for (int x = tid - R; x < L.nx + R; x += M_GHOST_THREADS) {
+            for (int x = tid - L.gx; x < L.nx + L.gx; x += M_GHOST_THREADS) {
                 const int xs = x < 0 ? x + L.nx : (x >= L.nx ? x - L.nx : x);
                 E v = src[xs];
                 if (zs != z) v = vswap(v);
                 dst[x] = v;
             }
         } else {
-            // the 2 x 3 x-ghost cells of M_GHOST_ROWS_PER_TASK interior rows
-            const long r = (long)(task - nb_rows) * M_GHOST_ROWS_PER_TASK + tid / (2 * R);
-            const int j = tid % (2 * R);
-            if (tid < M_GHOST_ROWS_PER_TASK * 2 * R && r < (long)L.ny * L.nz) {
+            // the 2 x gx x-ghost cells of rows_per_task interior rows
+            const long r = (long)(task - nb_rows) * rows_per_task + tid / per_row;
+            const int j = tid % per_row;
+            if (tid < rows_per_task * per_row && r < (long)L.ny * L.nz) {
                 const int y = (int)(r % L.ny), z = (int)(r / L.ny);
-                const int x = j < R ? j - R : L.nx + j - R;
-                const int xs = j < R ? x + L.nx : x - L.nx;
+                const int x = j < L.gx ? j - L.gx : L.nx + j - L.gx;
+                const int xs = j < L.gx ? x + L.nx : x - L.nx;
                 f[L.idx(x, y, z)] = f[L.idx(xs, y, z)];
             }
         }

@@ -61,6 +61,16 @@ constexpr int Q_OFF_MISC = Q_OFF_BARS + Q_NBARS * 8;  // tensor-memory base addr
 constexpr int Q_SMEM_BYTES = Q_OFF_MISC + 16;
 static_assert(Q_SLOT_BYTES % 128 == 0 && Q_PSLOT_BYTES % 128 == 0, "TMA destinations must stay 128-byte aligned");
 static_assert(Q_SMEM_BYTES <= 232448, "exceeds the 227 KB of shared memory a CTA may use");
+// MIX build (tensor-product mixed derivatives, NEXT-4): four staged planes of in-plane first derivatives (rows -3 .. 18
+// of the 16 tile columns; U: d_x u_y, d_x u_x; A: d_x A_y, d_x A_x) take the place of the z phase table, which that
+// build reads from global memory; two more mbarriers per role order the staging.
+constexpr int Q_STAGE_FIELD = Q_WY * Q_TX;             // 352 elements
+constexpr int QX_OFF_STAGE = Q_OFF_ZTAB;
+constexpr int QX_OFF_BARS = QX_OFF_STAGE + 4 * Q_STAGE_FIELD * 8;
+constexpr int QX_NBARS = Q_NBARS + 4;                  // + staged / gathered, per role
+constexpr int QX_OFF_MISC = QX_OFF_BARS + QX_NBARS * 8;
+constexpr int QX_SMEM_BYTES = QX_OFF_MISC + 16;
+static_assert(QX_SMEM_BYTES <= 232448, "exceeds the 227 KB of shared memory a CTA may use");
 
 // tensor-memory columns (32-bit) of one lane; an 8-byte element takes two
 constexpr int Q_NH = 8;                        // history depth (planes p-6 .. p, one spare)
@@ -288,19 +298,69 @@ __device__ __forceinline__ void q_hist_gather(uint32_t base, int k, const E (&c1
     }
 }
 
+// ---- tensor-product mixed derivatives in the plane (MIX build; reading G2 alternative, NEXT-4) ------------------
+// D_x D_y f is taken as D_y (D_x f): every thread stages D_x f of its two cells, the role's 128 threads add the 2 x 3
+// halo rows above and below the tile (96 points per staged field, formed from the ring by the expression the owners
+// use, so that a grid point gets the same bits whoever computes it), and after the role's barrier each thread takes
+// the y derivative of its pair from the staged plane: 8 loads for two cells and one field, where the bidiagonal
+// stencil takes 20.  st points at the role's two staged fields; pa / pb at field a / b of the ring plane, row 0,
+// first tile column.
+template <typename E>
+__device__ __forceinline__ void q_stage(E* __restrict__ st, const E* __restrict__ pa, const E* __restrict__ pb, const E (&c1x)[3],
+                                        const E (&own_a)[2], const E (&own_b)[2], int rt, int wp, int lane, int tx, int ty0) {
+#pragma unroll
+    for (int cc = 0; cc < 2; cc++) {
+        st[(ty0 + R + cc) * Q_TX + tx] = own_a[cc];
+        st[Q_STAGE_FIELD + (ty0 + R + cc) * Q_TX + tx] = own_b[cc];
+    }
+    // halo points 0 .. 95 of field a, 96 .. 191 of field b: one each, then lanes 0 .. 15 of every warp a second one
+#pragma unroll
+    for (int pass = 0; pass < 2; pass++) {
+        const int item = pass == 0 ? rt : 128 + wp * 16 + lane;
+        if (pass == 0 || lane < 16) {
+            const bool second = item >= 96;
+            const int r = second ? item - 96 : item;
+            const int hrow = r >> 4, hx = r & 15;
+            const int row = hrow < R ? hrow : hrow + Q_TY;          // rows 0 1 2 and 19 20 21 of the 22 loaded
+            const E* hp = (second ? pb : pa) + row * Q_WX + hx;
+            E hd[3];
+#pragma unroll
+            for (int m = 1; m <= 3; m++) hd[m - 1] = vsub(hp[m], hp[-m]);
+            st[(second ? Q_STAGE_FIELD : 0) + row * Q_TX + hx] = m_dot3(c1x, hd);
+        }
+    }
+}
+// y differences of the staged field around the two cells of the pair
+template <typename E>
+__device__ __forceinline__ void q_stage_diff(const E* __restrict__ st, int tx, int ty0, E (&e)[2][3]) {
+    E col[8];
+#pragma unroll
+    for (int r = 0; r < 8; r++) col[r] = st[(ty0 + r) * Q_TX + tx];
+#pragma unroll
+    for (int m = 1; m <= 3; m++) {
+        e[0][m - 1] = vsub(col[3 + m], col[3 - m]);
+        e[1][m - 1] = vsub(col[4 + m], col[4 - m]);
+    }
+}
+
 // UPW: continuity equation with the 5th-order upwind correction (G17); the U role forms
 // sum_a |u_a| delta6_a ln rho / (60 h_a) itself (x, y parts parked, the z part scattered).
-template <typename T, bool UPW>
+// MIX: mixed derivatives as tensor products D_a (D_b f) instead of the bidiagonal stencil (ac_set_mixed(1)): the z-mixed
+// ones are the z stencil of an in-plane first derivative (scattered like every other z sum), the in-plane ones
+// go through q_stage.
+template <typename T, bool UPW, bool MIX = false>
 __global__ void __launch_bounds__(Q_THREADS, 1)
     substep_pair_kernel(const __grid_constant__ MarchArgs<T> a, const __grid_constant__ CUtensorMap map_in,
                         const __grid_constant__ CUtensorMap map_prev) {
     using E = typename ElemOf<T>::E;
     extern __shared__ __align__(1024) unsigned char smem[];
     E* ztab = (E*)(smem + Q_OFF_ZTAB);
-    uint64_t* full = (uint64_t*)(smem + Q_OFF_BARS);
+    uint64_t* full = (uint64_t*)(smem + (MIX ? QX_OFF_BARS : Q_OFF_BARS));
     uint64_t* done = full + Q_NP;
     uint64_t* mfull = done + Q_NP;            // [warp pair 0..3][depth]   A -> U mailbox (tensor memory)
-    uint32_t* tmem_word = (uint32_t*)(smem + Q_OFF_MISC);
+    uint64_t* staged = mfull + 4 * Q_ND;      // MIX: [role] the staged plane is complete; gathered = it may be overwritten
+    uint64_t* gathered = staged + 2;
+    uint32_t* tmem_word = (uint32_t*)(smem + (MIX ? QX_OFF_MISC : Q_OFF_MISC));
 
     const Layout& L = a.L;
     const MarchCoef<E>& c = a.c;
@@ -326,6 +386,8 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
             m_bar_init(&done[s], Q_WORKERS / 32);
         }
         for (int s = 0; s < 4 * Q_ND; s++) m_bar_init(&mfull[s], 1);
+        if (MIX)
+            for (int s = 0; s < 4; s++) m_bar_init(&staged[s], 4);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 9) {
@@ -335,7 +397,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     // z phase table of this chunk: (cos, sin)(k_z z + phase) per level, lanes = (z, z + nz/2) for packed pairs
-    if (a.has_forcing) {
+    if (!MIX && a.has_forcing) {
         const T* tz = a.ftab + 2 * L.nx + 2 * L.ny;
         for (int i = tid; i < ze - zs; i += Q_THREADS) {
             const int z = zs + i;
@@ -402,28 +464,44 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                     }
                 }
                 // ---- u_x: d_x, d_y; L_x own; D_xy u_x -> L_y; D_xz u_x -> L_z; d_z u_x from the history ----
-                q_load<E, true, true>(pl + 1 * Q_PLANE, f0, d, s, e, t, q);
+                q_load<E, true, !MIX>(pl + 1 * Q_PLANE, f0, d, s, e, t, q);
 #pragma unroll
                 for (int cc = 0; cc < 2; cc++) {
                     ux0[cc] = f0[cc];
                     Gxx[cc] = m_dot3(c.c1x, d[cc]);
                     Gxy[cc] = m_dot3(c.c1y, e[cc]);
-                    lyip[cc] = m_dot3(c.cm3xy, q[cc]);
+                    if (!MIX) lyip[cc] = m_dot3(c.cm3xy, q[cc]);
                     Q_FIRST(Lx[cc], fLx[cc], c.w2z[0], c.w2z[0], f0[cc], f0[cc], f0[cc],
                             m_dot3(c.w2y[0], t[cc], m_dot3(c.w2x[0], s[cc], vfma(c.w20[0], f0[cc], Lx[cc][3]))));
-                    Q_FIRST(Lz[cc], fLz[cc], c.cm3xz, c.ncm3xz, d[cc][0], d[cc][1], d[cc][2], Lz[cc][3]);
+                    if (!MIX) Q_FIRST(Lz[cc], fLz[cc], c.cm3xz, c.ncm3xz, d[cc][0], d[cc][1], d[cc][2], Lz[cc][3]);
                 }
                 // ---- u_y: d_x, d_y; L_y own; D_xy u_y -> L_x; D_yz u_y -> L_z; d_z u_y from the history ----
-                q_load<E, true, true>(pl + 2 * Q_PLANE, f0, d, s, e, t, q);
+                q_load<E, true, !MIX>(pl + 2 * Q_PLANE, f0, d, s, e, t, q);
                 q_st4<E>(tm + Q_TM_UH + 8 + (uint32_t)((k & (Q_NH - 1)) * Q_UH_SLOT), ux0[0], ux0[1], f0[0], f0[1]);
 #pragma unroll
                 for (int cc = 0; cc < 2; cc++) {
                     Gyx[cc] = m_dot3(c.c1x, d[cc]);
                     Gyy[cc] = m_dot3(c.c1y, e[cc]);
-                    Lx[cc][2] = m_dot3(c.cm3xy, q[cc], Lx[cc][2]);
-                    Q_FIRST(Ly[cc], fLy[cc], c.w2z[1], c.w2z[1], f0[cc], f0[cc], f0[cc],
-                            m_dot3(c.w2y[1], t[cc], m_dot3(c.w2x[1], s[cc], vfma(c.w20[1], f0[cc], vadd(Ly[cc][3], lyip[cc])))));
-                    Q_NEXT(Lz[cc], fLz[cc], c.cm3yz, c.ncm3yz, e[cc][0], e[cc][1], e[cc][2]);
+                    if (!MIX) {
+                        Lx[cc][2] = m_dot3(c.cm3xy, q[cc], Lx[cc][2]);
+                        Q_FIRST(Ly[cc], fLy[cc], c.w2z[1], c.w2z[1], f0[cc], f0[cc], f0[cc],
+                                m_dot3(c.w2y[1], t[cc], m_dot3(c.w2x[1], s[cc], vfma(c.w20[1], f0[cc], vadd(Ly[cc][3], lyip[cc])))));
+                        Q_NEXT(Lz[cc], fLz[cc], c.cm3yz, c.ncm3yz, e[cc][0], e[cc][1], e[cc][2]);
+                    } else {
+                        // 1/3 d_z (d_x u_x + d_y u_y) -> L_z
+                        Q_FIRST(Ly[cc], fLy[cc], c.w2z[1], c.w2z[1], f0[cc], f0[cc], f0[cc],
+                                m_dot3(c.w2y[1], t[cc], m_dot3(c.w2x[1], s[cc], vfma(c.w20[1], f0[cc], Ly[cc][3]))));
+                        const E dxy = vadd(Gxx[cc], Gyy[cc]);
+                        Q_FIRST(Lz[cc], fLz[cc], c.c13z, c.nc13z, dxy, dxy, dxy, Lz[cc][3]);
+                    }
+                }
+                if (MIX) {
+                    // stage d_x u_y (-> L_x) and d_x u_x (-> L_y) once the role has finished with the previous plane
+                    if (k > 0) m_bar_wait<0>(&gathered[0], (uint32_t)((k - 1) & 1));
+                    q_stage<E>((E*)(smem + QX_OFF_STAGE), pl - cell_off + 2 * Q_PLANE + Q_HX, pl - cell_off + 1 * Q_PLANE + Q_HX,
+                               c.c1x, Gyx, Gxx, tid & 127, wp, lane, tx, ty0);
+                    __syncwarp();
+                    if (lane == 0) m_bar_arrive(&staged[0]);
                 }
                 // ---- u_z: d_x, d_y, d_z; L_z own; D_xz u_z -> L_x; D_yz u_z -> L_y ----
                 q_load<E, true, false>(pl + 3 * Q_PLANE, f0, d, s, e, t, q);
@@ -434,8 +512,28 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                     Gzy[cc] = m_dot3(c.c1y, e[cc]);
                     Q_NEXT(Lz[cc], fLz[cc], c.w2z[2], c.w2z[2], f0[cc], f0[cc], f0[cc]);
                     Lz[cc][2] = m_dot3(c.w2y[2], t[cc], m_dot3(c.w2x[2], s[cc], vfma(c.w20[2], f0[cc], Lz[cc][2])));
-                    Q_NEXT(Lx[cc], fLx[cc], c.cm3xz, c.ncm3xz, d[cc][0], d[cc][1], d[cc][2]);
-                    Q_NEXT(Ly[cc], fLy[cc], c.cm3yz, c.ncm3yz, e[cc][0], e[cc][1], e[cc][2]);
+                    if (!MIX) {
+                        Q_NEXT(Lx[cc], fLx[cc], c.cm3xz, c.ncm3xz, d[cc][0], d[cc][1], d[cc][2]);
+                        Q_NEXT(Ly[cc], fLy[cc], c.cm3yz, c.ncm3yz, e[cc][0], e[cc][1], e[cc][2]);
+                    } else {
+                        // 1/3 d_z (d_x u_z) -> L_x, 1/3 d_z (d_y u_z) -> L_y
+                        Q_NEXT(Lx[cc], fLx[cc], c.c13z, c.nc13z, Gzx[cc], Gzx[cc], Gzx[cc]);
+                        Q_NEXT(Ly[cc], fLy[cc], c.c13z, c.nc13z, Gzy[cc], Gzy[cc], Gzy[cc]);
+                    }
+                }
+                if (MIX) {
+                    // 1/3 d_y (d_x u_y) -> L_x, 1/3 d_y (d_x u_x) -> L_y of this plane (level 3 sits in slot 2)
+                    m_bar_wait<0>(&staged[0], (uint32_t)(k & 1));
+                    const E* st = (const E*)(smem + QX_OFF_STAGE);
+                    E ey[2][3];
+                    q_stage_diff<E>(st, tx, ty0, ey);
+#pragma unroll
+                    for (int cc = 0; cc < 2; cc++) Lx[cc][2] = m_dot3(c.c13y, ey[cc], Lx[cc][2]);
+                    q_stage_diff<E>(st + Q_STAGE_FIELD, tx, ty0, ey);
+#pragma unroll
+                    for (int cc = 0; cc < 2; cc++) Ly[cc][2] = m_dot3(c.c13y, ey[cc], Ly[cc][2]);
+                    __syncwarp();
+                    if (lane == 0) m_bar_arrive(&gathered[0]);
                 }
                 // ---- park the in-plane first derivatives of this plane (needed when it is finalised, 3 iterations on) ----
 #pragma unroll
@@ -574,7 +672,8 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                 E fPz[2], fJx[2], fJy[2], fJz[2];
                 E Bz[2], Bxip[2], Byip[2], Pxip[2], Pyip[2], jxip[2], jyip[2], ax0[2];
                 // ---- A_x: B_z -= d_y A_x; in-plane lap; J_x -= D_yy A_x; D_xy A_x -> J_y; D_xz A_x -> J_z; d_z, d_zz from the history
-                q_load<E, true, true>(pl + 4 * Q_PLANE, f0, d, s, e, t, q);
+                E dxax[2], dxay[2];    // MIX only
+                q_load<E, true, !MIX>(pl + 4 * Q_PLANE, f0, d, s, e, t, q);
 #pragma unroll
                 for (int cc = 0; cc < 2; cc++) {
                     ax0[cc] = f0[cc];
@@ -582,20 +681,41 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                     const E px = m_dot3(c.c2x, s[cc]), py = m_dot3(c.c2y, t[cc]);
                     Pxip[cc] = vadd(vfma(c20xy, f0[cc], px), py);
                     jxip[cc] = vneg(vfma(c.c20y, f0[cc], py));
-                    jyip[cc] = m_dot3(c.cmxy, q[cc]);
-                    Q_FIRST(Jz[cc], fJz[cc], c.cmxz, c.ncmxz, d[cc][0], d[cc][1], d[cc][2], Jz[cc][3]);
+                    if (!MIX) {
+                        jyip[cc] = m_dot3(c.cmxy, q[cc]);
+                        Q_FIRST(Jz[cc], fJz[cc], c.cmxz, c.ncmxz, d[cc][0], d[cc][1], d[cc][2], Jz[cc][3]);
+                    } else {
+                        dxax[cc] = m_dot3(c.c1x, d[cc]);
+                    }
                 }
                 // ---- A_y: B_z += d_x A_y; in-plane lap; J_y -= D_xx A_y; D_xy A_y -> J_x; D_yz A_y -> J_z; d_z, d_zz from the history
-                q_load<E, true, true>(pl + 5 * Q_PLANE, f0, d, s, e, t, q);
+                q_load<E, true, !MIX>(pl + 5 * Q_PLANE, f0, d, s, e, t, q);
                 q_st4<E>(tm + Q_TM_AH + (uint32_t)((k & (Q_NH - 1)) * Q_AH_SLOT), ax0[0], ax0[1], f0[0], f0[1]);
 #pragma unroll
                 for (int cc = 0; cc < 2; cc++) {
-                    Bz[cc] = m_dot3(c.c1x, d[cc], Bz[cc]);
                     const E px = m_dot3(c.c2x, s[cc]), py = m_dot3(c.c2y, t[cc]);
                     Pyip[cc] = vadd(vfma(c20xy, f0[cc], px), py);
-                    jyip[cc] = vsub(jyip[cc], vfma(c.c20x, f0[cc], px));
-                    jxip[cc] = m_dot3(c.cmxy, q[cc], jxip[cc]);
-                    Q_NEXT(Jz[cc], fJz[cc], c.cmyz, c.ncmyz, e[cc][0], e[cc][1], e[cc][2]);
+                    if (!MIX) {
+                        Bz[cc] = m_dot3(c.c1x, d[cc], Bz[cc]);
+                        jyip[cc] = vsub(jyip[cc], vfma(c.c20x, f0[cc], px));
+                        jxip[cc] = m_dot3(c.cmxy, q[cc], jxip[cc]);
+                        Q_NEXT(Jz[cc], fJz[cc], c.cmyz, c.ncmyz, e[cc][0], e[cc][1], e[cc][2]);
+                    } else {
+                        dxay[cc] = m_dot3(c.c1x, d[cc]);
+                        Bz[cc] = vadd(Bz[cc], dxay[cc]);
+                        jyip[cc] = vneg(vfma(c.c20x, f0[cc], px));
+                        // d_z (d_x A_x + d_y A_y) -> J_z
+                        const E dxy = vadd(dxax[cc], m_dot3(c.c1y, e[cc]));
+                        Q_FIRST(Jz[cc], fJz[cc], c.c1z, c.nc1z, dxy, dxy, dxy, Jz[cc][3]);
+                    }
+                }
+                if (MIX) {
+                    // stage d_x A_y (-> J_x) and d_x A_x (-> J_y)
+                    if (k > 0) m_bar_wait<0>(&gathered[1], (uint32_t)((k - 1) & 1));
+                    q_stage<E>((E*)(smem + QX_OFF_STAGE) + 2 * Q_STAGE_FIELD, pl - cell_off + 5 * Q_PLANE + Q_HX,
+                               pl - cell_off + 4 * Q_PLANE + Q_HX, c.c1x, dxay, dxax, tid & 127, wp, lane, tx, ty0);
+                    __syncwarp();
+                    if (lane == 0) m_bar_arrive(&staged[1]);
                 }
                 // ---- A_z: B_x += d_y A_z; B_y -= d_x A_z; lap; J_z -= (D_xx + D_yy) A_z; D_xz A_z -> J_x; D_yz A_z -> J_y
                 q_load<E, true, false>(pl + 6 * Q_PLANE, f0, d, s, e, t, q);
@@ -606,8 +726,29 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                     const E pxy = vadd(m_dot3(c.c2x, s[cc]), m_dot3(c.c2y, t[cc]));
                     Jz[cc][2] = vsub(vfma(c.nc20xy, f0[cc], Jz[cc][2]), pxy);
                     Q_FIRST(Pz[cc], fPz[cc], c.c2z, c.c2z, f0[cc], f0[cc], f0[cc], vadd(vfma(c.c20all, f0[cc], Pz[cc][3]), pxy));
-                    Q_FIRST(Jx[cc], fJx[cc], c.cmxz, c.ncmxz, d[cc][0], d[cc][1], d[cc][2], vadd(Jx[cc][3], jxip[cc]));
-                    Q_FIRST(Jy[cc], fJy[cc], c.cmyz, c.ncmyz, e[cc][0], e[cc][1], e[cc][2], vadd(Jy[cc][3], jyip[cc]));
+                    if (!MIX) {
+                        Q_FIRST(Jx[cc], fJx[cc], c.cmxz, c.ncmxz, d[cc][0], d[cc][1], d[cc][2], vadd(Jx[cc][3], jxip[cc]));
+                        Q_FIRST(Jy[cc], fJy[cc], c.cmyz, c.ncmyz, e[cc][0], e[cc][1], e[cc][2], vadd(Jy[cc][3], jyip[cc]));
+                    } else {
+                        // d_z (d_x A_z) -> J_x, d_z (d_y A_z) -> J_y
+                        const E dxaz = vneg(Byip[cc]), dyaz = Bxip[cc];
+                        Q_FIRST(Jx[cc], fJx[cc], c.c1z, c.nc1z, dxaz, dxaz, dxaz, vadd(Jx[cc][3], jxip[cc]));
+                        Q_FIRST(Jy[cc], fJy[cc], c.c1z, c.nc1z, dyaz, dyaz, dyaz, vadd(Jy[cc][3], jyip[cc]));
+                    }
+                }
+                if (MIX) {
+                    // d_y (d_x A_y) -> J_x, d_y (d_x A_x) -> J_y of this plane (level 3 sits in slot 2)
+                    m_bar_wait<0>(&staged[1], (uint32_t)(k & 1));
+                    const E* st = (const E*)(smem + QX_OFF_STAGE) + 2 * Q_STAGE_FIELD;
+                    E ey[2][3];
+                    q_stage_diff<E>(st, tx, ty0, ey);
+#pragma unroll
+                    for (int cc = 0; cc < 2; cc++) Jx[cc][2] = m_dot3(c.c1y, ey[cc], Jx[cc][2]);
+                    q_stage_diff<E>(st + Q_STAGE_FIELD, tx, ty0, ey);
+#pragma unroll
+                    for (int cc = 0; cc < 2; cc++) Jy[cc][2] = m_dot3(c.c1y, ey[cc], Jy[cc][2]);
+                    __syncwarp();
+                    if (lane == 0) m_bar_arrive(&gathered[1]);
                 }
 #pragma unroll
                 for (int cc = 0; cc < 2; cc++) {
@@ -626,8 +767,15 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                     q_hist_gather<E, true, Q_AH_SLOT>(tm + Q_TM_AH, k, c.c1z, c.c2z, c.c20z, dzax, dzay, zzax, zzay, axc, ayc);
                     E cz_ = vzero<E>(), sz_ = vzero<E>();
                     if (a.has_forcing) {
-                        cz_ = ztab[2 * (z - zs)];
-                        sz_ = ztab[2 * (z - zs) + 1];
+                        if (MIX) {
+                            const T* tz = a.ftab + 2 * L.nx + 2 * L.ny;
+                            const int z2 = (ElemOf<T>::LANES == 2) ? z + L.nz : z;
+                            cz_ = vmake(tz[z], tz[z2]);
+                            sz_ = vmake(tz[a.nz_full + z], tz[a.nz_full + z2]);
+                        } else {
+                            cz_ = ztab[2 * (z - zs)];
+                            sz_ = ztab[2 * (z - zs) + 1];
+                        }
                     }
                     E b0[2], b1[2], b2[2], P0[2], P1[2];
 #pragma unroll

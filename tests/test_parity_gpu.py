@@ -419,30 +419,66 @@ def test_s9_reductions_match_the_oracle_on_ragged_grids(variant, shape):
     assert abs(d1["dt_cfl"] - dt) <= 1e-12 * dt
 
 
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("upwind", [False, True])
 @pytest.mark.parametrize("dtype", [binding.AC_F64, binding.AC_F32])
-def test_next4_tensor_product_mixed_reading(dtype):
-    """NEXT-4 (reading G2's alternative): ac_set_mixed("tensor") against the oracle's mixed="tensor" flag; the two
-    readings differ at truncation level, far above the parity tolerance, so the flag is shown to take effect."""
+def test_next4_tensor_product_mixed_reading(dtype, upwind, variant):
+    """NEXT-4 (reading G2's alternative): ac_set_mixed("tensor") against the oracle's mixed="tensor" flag, in the
+    pair-march kernel (variant 0: staged in-plane first derivatives, the performance variant) and in the direct
+    kernel; the two readings differ at truncation level, far above the parity tolerance, so the flag is shown to take
+    effect.  Three steps: every substep kind, the previous-state ring and the staging barriers over many planes; the
+    grid is ragged in y (40 = 2.5 tiles)."""
     shape = (24, 40, 32)
     lengths = (2 * math.pi, 1.6 * math.pi, 2.2 * math.pi)
     npdt = np.float64 if dtype == binding.AC_F64 else np.float32
     state = inputs.smooth_strong_state(shape, 31).astype(npdt)
     nu, eta, dt = 2e-2, 1e-2, 2e-3
-    ctx = make_ctx(shape, dtype=dtype, lengths=lengths, nu=nu, eta=eta, k_f=3, helicity=1.0)
+    ctx = make_ctx(shape, dtype=dtype, lengths=lengths, nu=nu, eta=eta, k_f=3, helicity=1.0, variant=variant)
     ctx.ac_set_mixed("tensor")
+    ctx.ac_set_upwind(upwind)
     ctx.ac_load_state(state)
-    f = helpers.oracle_forcing(9, 0, 3, 1.0, dt, 0.02, 1.0, lengths)
-    ctx.ac_step(dt, ctx.ac_make_forcing(9, 0, dt, 0.02))
+    want = state.astype(np.float64)
+    other = want
+    n0 = ctx.ac_launch_count()
+    for s in range(3):
+        f = helpers.oracle_forcing(9, s, 3, 1.0, dt, 0.02, 1.0, lengths)
+        ctx.ac_step(dt, ctx.ac_make_forcing(9, s, dt, 0.02))
+        want = mhd_c.step(want, dt, lengths, nu, eta, 1.0, f, mixed="tensor", upwind=upwind)
+        other = mhd_c.step(other, dt, lengths, nu, eta, 1.0, f, mixed="bidiagonal", upwind=upwind)
+        if s == 0:
+            n1 = ctx.ac_launch_count()
+            err1 = helpers.max_group_error(ctx.ac_store_state(), want)
     got = ctx.ac_store_state()
     ctx.ac_free()
-    s64 = state.astype(np.float64)
-    want = mhd_c.step(s64, dt, lengths, nu, eta, 1.0, f, mixed="tensor")
-    other = mhd_c.step(s64, dt, lengths, nu, eta, 1.0, f, mixed="bidiagonal")
     err = helpers.max_group_error(got, want)
     gap = helpers.max_group_error(other, want)
-    print("tensor-product mixed parity", npdt.__name__, err, "tensor vs bidiagonal", gap)
-    assert err <= (1e-12 if dtype == binding.AC_F64 else 1e-5)
+    print("tensor-product mixed parity", npdt.__name__, "variant", variant, "upwind", upwind, "1 step", err1, "3 steps", err,
+          "tensor vs bidiagonal", gap)
+    assert err1 <= (1e-12 if dtype == binding.AC_F64 else 1e-5)
+    assert err <= (3e-12 if dtype == binding.AC_F64 else 3e-5)
     assert gap > 100 * err or dtype == binding.AC_F32
+    if variant == 0:
+        assert n1 - n0 == 7               # the march path: forcing tables + 3 x (substep + ghost zones)
+
+
+@pytest.mark.parametrize("dtype", [binding.AC_F64, binding.AC_F32])
+def test_next4_tensor_product_translation_invariance_is_bitwise(dtype):
+    """P14 for the staged tensor-product build of the pair-march kernel: a staged derivative has the same bits
+    whether a tile's owner thread or a neighbour tile's halo thread formed it."""
+    shape = (40, 36, 64)
+    npdt = np.float64 if dtype == binding.AC_F64 else np.float32
+    state = inputs.smooth_strong_state(shape, 22).astype(npdt)
+    ctx = make_ctx(shape, dtype=dtype, nu=2e-3, eta=3e-3, variant=0)
+    ctx.ac_set_mixed("tensor")
+    outs = []
+    for shift in ((0, 0, 0), (7, 5, 13), (-3, 17, 31)):
+        rolled = np.ascontiguousarray(np.roll(state, shift, axis=(1, 2, 3)))
+        ctx.ac_load_state(rolled)
+        for s in range(2):
+            ctx.ac_step(1e-3, None)
+        outs.append(np.roll(ctx.ac_store_state(), tuple(-s for s in shift), axis=(1, 2, 3)))
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+    ctx.ac_free()
 
 
 def test_per_field_load_store_and_option_errors():

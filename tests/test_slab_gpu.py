@@ -53,6 +53,35 @@ def test_slabs_equal_single_context(world, dtype, variant, overlap):
     grp.free()
 
 
+@pytest.mark.parametrize("dtype", [binding.AC_F64, binding.AC_F32])
+def test_slabs_with_the_tensor_product_reading(dtype):
+    """The NEXT-4 build of the pair-march kernel (ac_set_mixed("tensor")) through the inner / outer split: its staged
+    planes and their barriers must not care where a launch starts and ends along z."""
+    shape = (48, 24, 32)
+    lengths = (2 * math.pi, 1.5 * math.pi, 3.0 * math.pi)
+    npdt = np.float64 if dtype == binding.AC_F64 else np.float32
+    state = inputs.smooth_strong_state(shape, 43).astype(npdt)
+    kw = dict(nu=5e-3, eta=4e-3, cs=1.0, k_f=3, helicity=1.0)
+
+    def tensor_context(*a, **k):
+        ctx = binding.Context(*a, **k)
+        ctx.ac_set_mixed("tensor")
+        return ctx
+
+    one = tensor_context(shape, lengths, dtype, **kw)
+    grp = slab.SlabGroupInProcess(shape, lengths, 2, dtype, variant=0, overlap=True, context_factory=tensor_context, **kw)
+    one.ac_load_state(state)
+    grp.load_state(state)
+    n0 = one.ac_launch_count()
+    for _ in range(2):
+        one.ac_step(2e-3, None)
+        grp.step(2e-3, None)
+    assert one.ac_launch_count() - n0 == 12           # the march path (substep + ghost zones), not the direct kernel
+    assert np.array_equal(one.ac_store_state(), grp.store_state())
+    one.ac_free()
+    grp.free()
+
+
 def test_three_substeps_equal_one_step():
     shape = (16, 24, 32)
     state = inputs.smooth_strong_state(shape, 5)
