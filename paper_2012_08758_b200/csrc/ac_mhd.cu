@@ -623,6 +623,8 @@ int configure(ac_ctx* ctx) {
     ctx->packed = ctx->march && ctx->dtype == AC_F32;
     ctx->L = layout_for(g, ctx->dtype, ctx->packed);
     ctx->cv = carve(ctx->L, store_elem_size(ctx->dtype, ctx->packed), elem_size(ctx->dtype), g->nz);
+    // the pair-march kernel addresses its stores with 32-bit element offsets (1024^3 padded: 1.1e9 elements per field)
+    if (ctx->march && ctx->variant == 0 && ctx->L.field > 0xffffffffull) return AC_EINVAL;
     ctx->loaded = false;
     ctx->loaded_mask = 0;
     ctx->cur = 0;

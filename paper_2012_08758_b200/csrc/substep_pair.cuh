@@ -440,6 +440,9 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(M_REGS_WORKER));
         const bool valid_x = x < L.nx;
+        // element index of the pair's first cell in the plane finalised next: a running 32-bit offset (a padded field has
+        // fewer than 2^32 elements, checked by the host) instead of Layout::idx() from scratch for every store
+        uint32_t out_idx = (uint32_t)L.idx(x, y, zs);
         if (warp < 4) {
             // =============================== U: ln rho, u ===============================
             E Lx[2][6], Ly[2][6], Lz[2][6], u6z[2][6];
@@ -633,7 +636,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                         o2 = vfma(c.rk_b, r1, o2);
                         o3 = vfma(c.rk_b, r2, o3);
                         if (valid_x && y + cc < L.ny) {
-                            const size_t ci = L.idx(x, y + cc, z);
+                            const uint32_t ci = out_idx + (uint32_t)(cc * L.pitch);
                             a.out[0][ci] = o0;
                             a.out[1][ci] = o1;
                             a.out[2][ci] = o2;
@@ -641,6 +644,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                         }
                     }
                     q_fence_before();
+                    out_idx += (uint32_t)L.plane;
                 }
                 __syncwarp();
                 if (lane == 0) m_bar_arrive(&done[k % Q_NP]);
@@ -836,12 +840,13 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                         o1 = vfma(c.rk_b, r1, o1);
                         o2 = vfma(c.rk_b, r2, o2);
                         if (valid_x && y + cc < L.ny) {
-                            const size_t ci = L.idx(x, y + cc, z);
+                            const uint32_t ci = out_idx + (uint32_t)(cc * L.pitch);
                             a.out[4][ci] = o0;
                             a.out[5][ci] = o1;
                             a.out[6][ci] = o2;
                         }
                     }
+                    out_idx += (uint32_t)L.plane;
                 }
                 __syncwarp();
                 if (lane == 0) m_bar_arrive(&done[k % Q_NP]);
