@@ -50,7 +50,8 @@ typedef enum {
     AC_EINVAL = -1, /* NULL pointer, bad grid (n < 8, nx % 4 != 0), non-positive L or cs, negative nu/eta, bad dt */
     AC_ENOMEM = -2, /* device or host allocation failed / workspace too small */
     AC_ECUDA = -3,  /* CUDA error (sticky); text from ac_strerror(AC_ECUDA) on the same thread */
-    AC_ESTATE = -4  /* ac_step / ac_reduce / ac_store_state before ac_load_state; a call that is not allowed between substeps */
+    AC_ESTATE = -4, /* ac_step / ac_reduce / ac_store_state before ac_load_state; a call that is not allowed between substeps */
+    AC_ELIMIT = -5  /* ac_reduce_dense_noalloc: more than AC_NOALLOC_MAX_CELLS cells */
 } ac_status;
 
 /* Periodic box: n cells and side length per axis; spacing h_a = l_a / n_a (l = 2 pi). */
@@ -213,6 +214,35 @@ typedef struct {
 } ac_diag_ext;
 int ac_reduce_ext(ac_ctx* ctx, ac_diag_ext* out);
 int ac_reduce_ext_raw(ac_ctx* ctx, double out[3]);
+
+/* ac_reduce_dense_noalloc: the reductions of ac_reduce_raw WITHOUT a context and without any allocation, for callers
+ * that cannot call cudaMalloc (code under CUDA graph capture, serving loops, harnesses that forbid it).  It calls no
+ * cudaMalloc / cudaFree / cudaMallocHost and no allocating library routine, does no host <-> device copy and does not
+ * synchronise: two kernel launches on cuda_stream (NULL: the default stream) of the CURRENT device.
+ *   state_dev  DEVICE pointer, dense [7][nz][ny][nx] elements of dtype (float / double), x fastest, field order
+ *              ln rho, u_x, u_y, u_z, A_x, A_y, A_z: the array ac_load_state takes.  No ghost zones: the periodic
+ *              wrap is taken by index.  Read only; owned by the caller.
+ *   grid       as for ac_init (n >= 8 per axis, nx % 4 == 0); bext: uniform imposed field added to curl A, or NULL.
+ *   raw_dev    DEVICE pointer to 6 doubles (8-byte aligned), written by the second launch: {sum |u|^2, max |u|^2,
+ *              sum |B|^2, max |B|^2, min ln rho, max ln rho} with B = curl A + B_ext (6th-order first derivatives,
+ *              PAPER.md:85, 119; G1), i.e. ac_reduce_raw's six numbers; ac_diag_combine (nranks = 1) turns a host copy
+ *              of them into rms / max values and the CFL step (G15).  Per cell the arithmetic is that of ac_reduce,
+ *              so the maxima equal ac_reduce_raw's bit for bit, the sums to summation order (deterministic: fixed
+ *              two-stage tree); a non-finite ln rho or A makes sum |u|^2 non-finite.
+ * Scratch: the per-block partials live in a fixed array inside the library (static __device__, 3 MiB, held by every GPU
+ * that loads the library until the process exits), so the size is LIMITED: at most AC_NOALLOC_MAX_CELLS = 2^27 cells
+ * (512^3, BASELINE config 4; ac_noalloc_max_cells() returns it); more returns AC_ELIMIT and launches nothing.  Every
+ * call on a device shares that array and finds the previous call's partials in it; a call writes every partial it reads,
+ * so nothing has to be cleared - but two calls that overlap on the GPU (different streams of one device, or different
+ * host threads without ordering) RACE on it: order them on one stream or with events.  The first call on each device
+ * looks the array's device address up (cudaGetSymbolAddress; no allocation): under graph capture make one call on the
+ * device before the capture begins.
+ * Errors: AC_EINVAL (NULL / misaligned / non-device pointers, pointers of another device, bad grid or dtype, non-finite
+ * bext), AC_ELIMIT, AC_ECUDA. */
+#define AC_NOALLOC_MAX_CELLS (1LL << 27)
+int ac_reduce_dense_noalloc(const void* state_dev, ac_dtype dtype, const ac_grid* grid, const double bext[3],
+                            double* raw_dev, void* cuda_stream);
+long long ac_noalloc_max_cells(void);
 
 /* Host helpers for Eq. 4-6 (no device work).
  * ac_forcing_from_draws: u1, u2, u3 in [0, 1) choose the shell vector (index floor(u1*len) into

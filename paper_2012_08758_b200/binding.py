@@ -22,7 +22,7 @@ EXPORTS = (
     "ac_set_upwind", "ac_set_mixed", "ac_substep", "ac_state_layout", "ac_field_device_ptr", "ac_reduce_raw",
     "ac_reduce_ext", "ac_reduce_ext_raw", "ac_set_slab", "ac_substep_part", "ac_halo_bytes", "ac_halo_pack",
     "ac_halo_unpack", "ac_diag_combine", "ac_set_forcing_mode", "ac_halo_pull", "ac_workspace_ptr", "ac_ipc_export",
-    "ac_ipc_open", "ac_ipc_close",
+    "ac_ipc_open", "ac_ipc_close", "ac_reduce_dense_noalloc", "ac_noalloc_max_cells",
     "ac_launch_count", "ac_free", "ac_strerror", "ac_version",
 )
 
@@ -146,6 +146,10 @@ def load_library():
     L.ac_halo_unpack.restype = i32
     L.ac_diag_combine.argtypes = [vp, ctypes.POINTER(dbl), i32, ctypes.POINTER(AcDiag)]
     L.ac_diag_combine.restype = i32
+    L.ac_reduce_dense_noalloc.argtypes = [vp, i32, ctypes.POINTER(AcGrid), ctypes.POINTER(dbl), vp, vp]
+    L.ac_reduce_dense_noalloc.restype = i32
+    L.ac_noalloc_max_cells.argtypes = []
+    L.ac_noalloc_max_cells.restype = ctypes.c_longlong
     L.ac_launch_count.argtypes = [vp]
     L.ac_launch_count.restype = ctypes.c_longlong
     L.ac_free.argtypes = [vp]
@@ -194,6 +198,36 @@ def ac_ipc_open(handle):
 
 def ac_ipc_close(ptr):
     _check(load_library().ac_ipc_close(ctypes.c_void_p(ptr)), "ac_ipc_close")
+
+
+def ac_noalloc_max_cells():
+    return int(load_library().ac_noalloc_max_cells())
+
+
+def ac_reduce_dense_noalloc(state, lengths, raw_out, bext=None, stream=None):
+    """The reductions of ac_reduce_raw of a dense DEVICE state (torch CUDA tensor (7, nz, ny, nx), float32 or float64,
+    contiguous) into raw_out (torch CUDA tensor of 6 float64), without a context and without any allocation inside the
+    library (include/ac_mhd.h: at most ac_noalloc_max_cells() cells, calls must not overlap on the GPU).  Launches on
+    `stream` (a torch stream; None: torch's current stream) and returns without synchronising.  Marshalling only."""
+    import torch
+    if not (isinstance(state, torch.Tensor) and isinstance(raw_out, torch.Tensor) and state.is_cuda and raw_out.is_cuda):
+        raise AcError("ac_reduce_dense_noalloc takes CUDA tensors (no CPU fallback)")
+    if state.dim() != 4 or state.shape[0] != 7 or not state.is_contiguous():
+        raise AcError("state must be a contiguous (7, nz, ny, nx) tensor")
+    if state.dtype not in (torch.float32, torch.float64):
+        raise AcError("state must be float32 or float64")
+    if raw_out.dtype != torch.float64 or raw_out.numel() != 6 or not raw_out.is_contiguous():
+        raise AcError("raw_out must be 6 contiguous float64")
+    if raw_out.device != state.device:
+        raise AcError("state and raw_out must live on the same device")
+    grid = _grid(tuple(state.shape[1:]), lengths)
+    dtype = AC_F64 if state.dtype == torch.float64 else AC_F32
+    b = (ctypes.c_double * 3)(*[float(v) for v in bext]) if bext is not None else None
+    with torch.cuda.device(state.device):
+        st = stream if stream is not None else torch.cuda.current_stream(state.device)
+        _check(load_library().ac_reduce_dense_noalloc(ctypes.c_void_p(state.data_ptr()), dtype, ctypes.byref(grid), b,
+                                                      ctypes.c_void_p(raw_out.data_ptr()),
+                                                      ctypes.c_void_p(st.cuda_stream)), "ac_reduce_dense_noalloc")
 
 
 def ac_version():

@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <type_traits>
 #include <vector>
@@ -19,6 +20,7 @@
 #include "kernels.cuh"
 #include "layout.cuh"
 #include "mhd_cell.cuh"
+#include "reduce_dense.cuh"
 #include "reduce_tma.cuh"
 #include "substep_march.cuh"
 #include "substep_pair.cuh"
@@ -1220,6 +1222,87 @@ void ac_free(ac_ctx* ctx) {
     delete ctx;
 }
 
+// ---- ac_reduce_dense_noalloc: the one entry point that allocates nothing ---------------------------------------
+// Its scratch memory (the per-block partials of reduce_dense_stage1_kernel) is this fixed array: every GPU that loads
+// the library holds its 3 MiB until the process exits.  In HOST code the name below is a host-side stand-in, not a
+// device address; the kernels get the address cudaGetSymbolAddress returns for the current device, looked up once per
+// device (noalloc_scratch) in this same file.
+}  // extern "C"
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[(size_t)ac::RD_MAX_PARTIALS * sizeof(ac::RedVals)];
+
+namespace {
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mutex;
+void* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};
+
+// device address of g_noalloc_scratch on the CURRENT device; set-up once per device, no allocation
+int noalloc_scratch(int dev, void** out) {
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        void* p = nullptr;
+        AC_CUDA(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        if (!p) return AC_ECUDA;
+        g_noalloc_ptr[dev] = p;
+    }
+    *out = g_noalloc_ptr[dev];
+    return AC_OK;
+}
+
+template <typename T>
+int reduce_dense_t(const void* state_dev, const ac_grid* g, const double bext[3], ac::RedVals* partial, double* raw_dev,
+                   cudaStream_t stream) {
+    ac::ReduceDenseArgs<T> a;
+    a.state = (const T*)state_dev;
+    a.nx = g->nx, a.ny = g->ny, a.nz = g->nz;
+    const double h[3] = {g->lx / g->nx, g->ly / g->ny, g->lz / g->nz};
+    for (int ax = 0; ax < 3; ax++)
+        for (int m = 0; m < 3; m++) a.c1[ax][m] = (T)(W1[m] / h[ax]);
+    for (int i = 0; i < 3; i++) a.bext[i] = (T)(bext ? bext[i] : 0.0);
+    const long long ncell = (long long)g->nx * g->ny * g->nz;
+    const int blocks = (int)((ncell + ac::RD_CELLS_PER_BLOCK - 1) / ac::RD_CELLS_PER_BLOCK);   // <= RD_MAX_PARTIALS
+    // every partial that stage 2 reads is written by stage 1 of this call: nothing in the scratch array has to start
+    // at zero, whatever the previous call left there
+    ac::reduce_dense_stage1_kernel<T><<<blocks, ac::RD_THREADS, 0, stream>>>(a, partial);
+    ac::reduce_stage2_kernel<<<1, 256, 0, stream>>>(partial, blocks, (ac::RedVals*)raw_dev);
+    AC_CUDA(cudaGetLastError());
+    return AC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ac_reduce_dense_noalloc(const void* state_dev, ac_dtype dtype, const ac_grid* grid, const double bext[3],
+                            double* raw_dev, void* cuda_stream) {
+    if (!state_dev || !raw_dev || ((uintptr_t)raw_dev % 8) != 0) return AC_EINVAL;
+    if (!grid_ok(grid) || (dtype != AC_F32 && dtype != AC_F64)) return AC_EINVAL;
+    if (bext && !(std::isfinite(bext[0]) && std::isfinite(bext[1]) && std::isfinite(bext[2]))) return AC_EINVAL;
+    if ((long long)grid->nx * grid->ny * grid->nz > ac::RD_MAX_CELLS) return AC_ELIMIT;
+    int dev = 0;
+    AC_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return AC_EINVAL;
+    // both pointers must be memory the current device owns (a host pointer would fault in the kernel, or silently
+    // read host memory where the GPU can reach it)
+    const void* ptrs[2] = {state_dev, raw_dev};
+    for (const void* p : ptrs) {
+        cudaPointerAttributes at;
+        AC_CUDA(cudaPointerGetAttributes(&at, p));
+        if (!(at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged) ||
+            (at.type == cudaMemoryTypeDevice && at.device != dev))
+            return AC_EINVAL;
+    }
+    void* scratch = nullptr;
+    const int rc = noalloc_scratch(dev, &scratch);
+    if (rc != AC_OK) return rc;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    return dtype == AC_F64 ? reduce_dense_t<double>(state_dev, grid, bext, (ac::RedVals*)scratch, raw_dev, stream)
+                           : reduce_dense_t<float>(state_dev, grid, bext, (ac::RedVals*)scratch, raw_dev, stream);
+}
+
+long long ac_noalloc_max_cells(void) { return ac::RD_MAX_CELLS; }
+
 const char* ac_strerror(int status) {
     switch (status) {
         case AC_OK: return "ok";
@@ -1227,6 +1310,7 @@ const char* ac_strerror(int status) {
         case AC_ENOMEM: return "out of memory or workspace too small";
         case AC_ECUDA: return g_cuda_err;
         case AC_ESTATE: return "no state loaded (call ac_load_state first)";
+        case AC_ELIMIT: return "grid larger than the fixed scratch array of ac_reduce_dense_noalloc (2^27 cells = 512^3)";
         default: return "unknown status";
     }
 }
