@@ -440,6 +440,10 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(M_REGS_WORKER));
         const bool valid_x = x < L.nx;
+        // fp64 build: which of the pair's two cells lie inside the grid, kept in a register (the empty asm stops the
+        // compiler from rebuilding the two bits from the block and thread ids for every plane)
+        uint32_t okm = (valid_x && y < L.ny ? 1u : 0u) | (valid_x && y + 1 < L.ny ? 2u : 0u);
+        if (ElemOf<T>::LANES == 1) asm volatile("" : "+r"(okm));
         // element index of the pair's first cell in the plane finalised next: a running 32-bit offset (a padded field has
         // fewer than 2^32 elements, checked by the host) instead of Layout::idx() from scratch for every store
         uint32_t out_idx = (uint32_t)L.idx(x, y, zs);
@@ -635,7 +639,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                         o1 = vfma(c.rk_b, r0, o1);
                         o2 = vfma(c.rk_b, r1, o2);
                         o3 = vfma(c.rk_b, r2, o3);
-                        if (valid_x && y + cc < L.ny) {
+                        if (ElemOf<T>::LANES == 1 ? (okm & (1u << cc)) != 0 : (valid_x && y + cc < L.ny)) {
                             const uint32_t ci = out_idx + (uint32_t)(cc * L.pitch);
                             a.out[0][ci] = o0;
                             a.out[1][ci] = o1;
@@ -839,7 +843,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                         o0 = vfma(c.rk_b, r0, o0);
                         o1 = vfma(c.rk_b, r1, o1);
                         o2 = vfma(c.rk_b, r2, o2);
-                        if (valid_x && y + cc < L.ny) {
+                        if (ElemOf<T>::LANES == 1 ? (okm & (1u << cc)) != 0 : (valid_x && y + cc < L.ny)) {
                             const uint32_t ci = out_idx + (uint32_t)(cc * L.pitch);
                             a.out[4][ci] = o0;
                             a.out[5][ci] = o1;
