@@ -406,9 +406,18 @@ int substep_t(ac_ctx* ctx, double dt, const ac_forcing* forcing, int s, int part
                 else if (ctx->upwind)
                     ac::substep_pair_kernel<T, true><<<gq, ac::Q_THREADS, ac::Q_SMEM_BYTES, ctx->stream>>>(
                         a, ctx->map_qin[ctx->cur], ctx->map_qprev[1 - ctx->cur]);
-                else
-                    ac::substep_pair_kernel<T, false><<<gq, ac::Q_THREADS, ac::Q_SMEM_BYTES, ctx->stream>>>(
-                        a, ctx->map_qin[ctx->cur], ctx->map_qprev[1 - ctx->cur]);
+                else {
+                    // the default build: previous-state and forcing switches fixed at compile time
+                    // (the forcing switch in the fp64 build only: it shortens the A role alone, which the packed
+                    // fp32 build cannot afford)
+                    constexpr int F1 = std::is_same<T, double>::value ? 1 : -1, F0 = std::is_same<T, double>::value ? 0 : -1;
+                    auto kern = s == 0 ? (forcing ? ac::substep_pair_kernel<T, false, false, 0, F1>
+                                                  : ac::substep_pair_kernel<T, false, false, 0, F0>)
+                                       : (forcing ? ac::substep_pair_kernel<T, false, false, 1, F1>
+                                                  : ac::substep_pair_kernel<T, false, false, 1, F0>);
+                    kern<<<gq, ac::Q_THREADS, ac::Q_SMEM_BYTES, ctx->stream>>>(a, ctx->map_qin[ctx->cur],
+                                                                                ctx->map_qprev[1 - ctx->cur]);
+                }
             } else {
                 dim3 grd((L.nx + ac::M_TX - 1) / ac::M_TX, (L.ny + ac::M_TY - 1) / ac::M_TY, nch);
                 if (ctx->upwind)
@@ -657,7 +666,7 @@ int configure(ac_ctx* ctx) {
         if (rc == AC_OK) rc = make_state_map(&ctx->map_qprev[b], ctx->field_ptr(b, 0), ctx->L, ac::Q_TX, ac::Q_TY);
         if (rc != AC_OK) return rc;
     }
-    const void* kernels[12] = {(const void*)ac::substep_march_kernel<double, false>,
+    const void* kernels[20] = {(const void*)ac::substep_march_kernel<double, false>,
                               (const void*)ac::substep_march_kernel<double, true>,
                               (const void*)ac::substep_march_kernel<float, false>,
                               (const void*)ac::substep_march_kernel<float, true>,
@@ -668,11 +677,19 @@ int configure(ac_ctx* ctx) {
                               (const void*)ac::substep_pair_kernel<double, false, true>,
                               (const void*)ac::substep_pair_kernel<double, true, true>,
                               (const void*)ac::substep_pair_kernel<float, false, true>,
-                              (const void*)ac::substep_pair_kernel<float, true, true>};
-    for (int k = 0; k < 12; k++) {
+                              (const void*)ac::substep_pair_kernel<float, true, true>,
+                              (const void*)ac::substep_pair_kernel<double, false, false, 0, 0>,
+                              (const void*)ac::substep_pair_kernel<double, false, false, 1, 0>,
+                              (const void*)ac::substep_pair_kernel<float, false, false, 0, -1>,
+                              (const void*)ac::substep_pair_kernel<float, false, false, 1, -1>,
+                              (const void*)ac::substep_pair_kernel<double, false, false, 0, 1>,
+                              (const void*)ac::substep_pair_kernel<double, false, false, 1, 1>,
+                              (const void*)ac::substep_pair_kernel<float, false, false, 0, -1>,
+                              (const void*)ac::substep_pair_kernel<float, false, false, 1, -1>};
+    for (int k = 0; k < 20; k++) {
         if ((ctx->dtype == AC_F64) != (k % 4 < 2)) continue;
         cudaError_t ea = cudaFuncSetAttribute(kernels[k], cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                              k < 4 ? ac::M_SMEM_BYTES : (k < 8 ? ac::Q_SMEM_BYTES : ac::QX_SMEM_BYTES));
+                                              k < 4 ? ac::M_SMEM_BYTES : (k < 8 || k >= 12 ? ac::Q_SMEM_BYTES : ac::QX_SMEM_BYTES));
         if (ea != cudaSuccess) return cuda_fail(ea, "cudaFuncSetAttribute(march kernel smem)");
     }
     // z chunks: every chunk re-reads 6 planes, every wave of CTAs costs (planes + 6) iterations;

@@ -348,7 +348,10 @@ __device__ __forceinline__ void q_stage_diff(const E* __restrict__ st, int tx, i
 // MIX: mixed derivatives as tensor products D_a (D_b f) instead of the bidiagonal stencil (ac_set_mixed(1)): the z-mixed
 // ones are the z stencil of an in-plane first derivative (scattered like every other z sum), the in-plane ones
 // go through q_stage.
-template <typename T, bool UPW, bool MIX = false>
+// PREV: -1 = the kernel reads MarchArgs::substep to see whether a previous state exists; 0 / 1 = fixed at compile time
+// (substep 0 / substeps 1, 2 of the default build: no uniform branches around the 2N-RK3 difference terms)
+// FORCE: the same for MarchArgs::has_forcing.
+template <typename T, bool UPW, bool MIX = false, int PREV = -1, int FORCE = -1>
 __global__ void __launch_bounds__(Q_THREADS, 1)
     substep_pair_kernel(const __grid_constant__ MarchArgs<T> a, const __grid_constant__ CUtensorMap map_in,
                         const __grid_constant__ CUtensorMap map_prev) {
@@ -378,7 +381,8 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
     const int ze = min(zs + a.cz, a.z_end);
     const int niter = ze - zs + 2 * R;      // planes zs-3 .. ze+2
     const int x = x0 + tx, y = y0 + ty0;
-    const bool with_prev = a.substep != 0;
+    const bool with_prev = PREV < 0 ? a.substep != 0 : PREV != 0;
+    const bool has_forcing = FORCE < 0 ? a.has_forcing != 0 : FORCE != 0;
 
     if (tid == 0) {
         for (int s = 0; s < Q_NP; s++) {
@@ -397,7 +401,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     // z phase table of this chunk: (cos, sin)(k_z z + phase) per level, lanes = (z, z + nz/2) for packed pairs
-    if (!MIX && a.has_forcing) {
+    if (!MIX && has_forcing) {
         const T* tz = a.ftab + 2 * L.nx + 2 * L.ny;
         for (int i = tid; i < ze - zs; i += Q_THREADS) {
             const int z = zs + i;
@@ -662,7 +666,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
 #pragma unroll
             for (int cc = 0; cc < 2; cc++) {
                 cxy[cc] = sxy[cc] = vzero<E>();
-                if (a.has_forcing && valid_x && y + cc < L.ny) {
+                if (has_forcing && valid_x && y + cc < L.ny) {
                     const T cx_ = a.ftab[x], sx_ = a.ftab[L.nx + x];
                     const T cy_ = a.ftab[2 * L.nx + y + cc], sy_ = a.ftab[2 * L.nx + L.ny + y + cc];
                     cxy[cc] = Splat<E>::of((double)(cx_ * cy_ - sx_ * sy_));
@@ -774,7 +778,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                     E dzax[2], dzay[2], zzax[2], zzay[2], axc[2], ayc[2];
                     q_hist_gather<E, true, Q_AH_SLOT>(tm + Q_TM_AH, k, c.c1z, c.c2z, c.c20z, dzax, dzay, zzax, zzay, axc, ayc);
                     E cz_ = vzero<E>(), sz_ = vzero<E>();
-                    if (a.has_forcing) {
+                    if (has_forcing) {
                         if (MIX) {
                             const T* tz = a.ftab + 2 * L.nx + 2 * L.ny;
                             const int z2 = (ElemOf<T>::LANES == 2) ? z + L.nz : z;
@@ -808,7 +812,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1)
                         E m0 = vmul(rho_inv, vsub(vmul(j1, b2[cc]), vmul(j2, b1[cc])));
                         E m1 = vmul(rho_inv, vsub(vmul(j2, b0[cc]), vmul(j0, b2[cc])));
                         E m2 = vmul(rho_inv, vsub(vmul(j0, b1[cc]), vmul(j1, b0[cc])));
-                        if (a.has_forcing) {
+                        if (has_forcing) {
                             // forcing Eq. 4: f_i = re_i cos(theta) - im_i sin(theta)
                             const E fc = vsub(vmul(cxy[cc], cz_), vmul(sxy[cc], sz_));
                             const E fs = vfma(sxy[cc], cz_, vmul(cxy[cc], sz_));
