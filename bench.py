@@ -258,8 +258,8 @@ def run_ours(args):
                          "kernel": "substep (avg of the 3 launches of a step)",
                          "note": "reported against HBM as BASELINE.json's metric asks; the kernel itself is limited by "
                                  "issue slots and the FP64 (fp32: packed FMA) pipe at two worker warps per scheduler "
-                                 "(59 % / 65 % busy, LSU pipe 76 %: profiles/r02_pair.md) and by the 1000 W power cap; "
-                                 "the ghost-zone kernel's time (3.7 %) is charged to the substep kernel",
+                                 "(61 % / 67 % busy, LSU pipe 80 %: profiles/r02_pair.md) and by the 1000 W power cap; "
+                                 "the ghost-zone kernel's time (3.9 %) is charged to the substep kernel",
                          "algorithmic_bytes_per_launch": alg_bytes_launch},
         }
         if do_e2e:
